@@ -1,0 +1,129 @@
+"""Pins P1, P2, P5: the oracle's radial functions against
+(a) closed-form values recorded in tests/golden/survey_pins.json and
+(b) their definitions as derivatives, evaluated with mpmath at 40 digits --
+neither route uses any oracle code."""
+import math
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+import oracle
+
+mp.mp.dps = 40
+
+
+def test_p1_bn_golden(golden):
+    g = golden["P1_ewald_bn"]
+    for case in g["cases"]:
+        got = oracle.ewald_bn(g["beta"], case["R"])
+        np.testing.assert_allclose(got, case["bn"], rtol=2e-13, atol=0)
+
+
+@pytest.mark.parametrize("R", [0.8, 0.9572, 1.7, 2.3, 4.4, 6.9])
+@pytest.mark.parametrize("beta", [0.5446, 0.31768, 0.9])
+def test_p1_bn_is_iterated_derivative(beta, R):
+    """bn_k = (-(1/R) d/dR)^k [erfc(beta R)/R]  (definition)."""
+    b = mp.mpf(beta)
+
+    def f0(r):
+        return mp.erfc(b * r) / r
+
+    def step(f):
+        return lambda r: -mp.diff(f, r) / r
+
+    fs = [f0]
+    for _ in range(3):
+        fs.append(step(fs[-1]))
+    want = [float(f(mp.mpf(R))) for f in fs]
+    got = oracle.ewald_bn(beta, R)
+    np.testing.assert_allclose(got, want, rtol=5e-12)
+
+
+@pytest.mark.parametrize("R", [0.5, 1.3, 7.0])
+def test_p1_beta_zero_is_bare_coulomb(R):
+    got = oracle.ewald_bn(0.0, R)
+    want = [1 / R, 1 / R**3, 3 / R**5, 15 / R**7]
+    np.testing.assert_allclose(got, want, rtol=1e-15)
+    # and the beta -> 0 limit of the screened form approaches it
+    near = oracle.ewald_bn(1e-4, R)
+    np.testing.assert_allclose(near[1:], want[1:], rtol=1e-9)
+
+
+def test_p2_lambda_golden(golden):
+    g = golden["P2_thole_lambda"]
+    for case in g["cases"]:
+        got = oracle.thole_lambda(g["a"], case["alpha"][0], case["alpha"][1], case["R"])
+        np.testing.assert_allclose(got, case["lambda"], rtol=2e-13)
+
+
+@pytest.mark.parametrize("R", [0.6, 0.9572, 1.5139, 2.4, 3.9])
+def test_p2_lambda_derivative_identities(R):
+    """lambda_5 = lambda_3 - R lambda_3'/3 ; lambda_7 = lambda_5 - R lambda_5'/5
+    (the three are successive radial derivatives of ONE damped kernel)."""
+    a, ai, aj = 0.39, 0.837, 0.496
+    c = mp.mpf(a) / mp.sqrt(mp.mpf(ai) * mp.mpf(aj))
+
+    def l3(r):
+        return 1 - mp.exp(-c * r**3)
+
+    def l5(r):
+        return l3(r) - r * mp.diff(l3, r) / 3
+
+    def l7(r):
+        return l5(r) - r * mp.diff(l5, r) / 5
+
+    want = [float(l3(mp.mpf(R))), float(l5(mp.mpf(R))), float(l7(mp.mpf(R)))]
+    got = oracle.thole_lambda(a, ai, aj, R)
+    np.testing.assert_allclose(got, want, rtol=1e-11, atol=1e-15)
+
+
+def test_p2_lambda_limits():
+    far = oracle.thole_lambda(0.39, 0.837, 0.496, 9.0)
+    np.testing.assert_allclose(far, [1, 1, 1], atol=1e-15)
+    near = oracle.thole_lambda(0.39, 0.837, 0.496, 1e-3)
+    assert np.all(np.abs(near) < 1e-8)
+    # symmetric in the two polarizabilities
+    np.testing.assert_array_equal(oracle.thole_lambda(0.39, 0.3, 1.7, 1.4),
+                                  oracle.thole_lambda(0.39, 1.7, 0.3, 1.4))
+
+
+def test_p5_masked_G_golden(golden):
+    g = golden["P5_masked_G"]
+    got = oracle.pair_G(g["beta"], g["a"], g["alpha"][0], g["alpha"][1], 0.0, g["R"])
+    np.testing.assert_allclose(got, g["G"], rtol=5e-13)
+    # masked branch is exactly bn_k - rr_k: no alpha dependence
+    other = oracle.pair_G(g["beta"], g["a"], 1.7, 0.31, 0.0, g["R"])
+    np.testing.assert_array_equal(got, other)
+
+
+def test_p4_G1_golden(golden):
+    g = golden["P4_charge_field"]
+    got = oracle.pair_G(g["beta"], g["a"], g["alpha"][0], g["alpha"][1], 1.0, g["R"])
+    assert math.isclose(got[0], g["G1"], rel_tol=5e-13)
+
+
+@pytest.mark.parametrize("s", [0.0, 1.0])
+@pytest.mark.parametrize("R", [0.9572, 1.6, 3.1, 6.5])
+def test_G_is_iterated_derivative_of_one_kernel(s, R):
+    """-f'/R = G1, -G1'/R = G2, -G2'/R = G3 with the scalar pair kernel
+    f(R) = erfc(bR)/R - 1/R + s g(R),  g = lambda_3/R + c^(1/3) Gamma(2/3, c R^3)
+    (g is the potential whose radial derivative gives lambda_3/R^2; (F4))."""
+    beta, a, ai, aj = 0.5446, 0.39, 0.837, 0.496
+    b = mp.mpf(beta)
+    c = mp.mpf(a) / mp.sqrt(mp.mpf(ai) * mp.mpf(aj))
+
+    def f(r):
+        x = c * r**3
+        g = (1 - mp.exp(-x)) / r + c ** (mp.mpf(1) / 3) * mp.gammainc(mp.mpf(2) / 3, x)
+        return mp.erfc(b * r) / r - 1 / r + s * g
+
+    def step(fn):
+        return lambda r: -mp.diff(fn, r) / r
+
+    g1 = step(f)
+    g2 = step(g1)
+    g3 = step(g2)
+    want = [float(g1(mp.mpf(R))), float(g2(mp.mpf(R))), float(g3(mp.mpf(R)))]
+    got = oracle.pair_G(beta, a, ai, aj, s, R)
+    np.testing.assert_allclose(got, want, rtol=2e-9, atol=1e-16)
