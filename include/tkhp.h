@@ -1,0 +1,190 @@
+/*
+ * tkhp.h -- C ABI of libtkhp: real-space AMOEBA polarization on one NVIDIA B200.
+ *
+ * Hot path of arXiv 2011.01207 (Tinker-HP on GPUs; "P:Lnnn" = PAPER.md line nnn):
+ *   blocked neighbour list  ->  permanent-multipole field  ->  induced-dipole
+ *   T.mu matrix-vector product inside a Jacobi-preconditioned CG solve  ->
+ *   polarization energy.
+ * The paper gives the organisation (32-atom groups and a group-pair list, P:L296-366;
+ * list filtering to a group->atom list with phantom atoms; pair kernels
+ * that compute every pair unscaled and apply the few scaling factors in a separate
+ * pass; PCG with a diagonal preconditioner, one polarization matrix-vector
+ * product per iteration; FP32 pair math with FP64 accumulation,
+ * P:L263-279).  It prints no interaction formula; the arithmetic is the standard
+ * AMOEBA real-space Ewald field with exponential Thole damping, written out in
+ * DESIGN.md section 2 (equations F1-F3, T1-T2, S, U), which restates SURVEY.md 8(c).
+ *
+ * Conventions (all entry points)
+ *   - Units: Angstrom, elementary charge, Angstrom^3; energy in kcal/mol.
+ *   - Every user-facing array is FP64, in ORIGINAL atom order (the spatial sort is
+ *     internal), C-contiguous.  Pointers named d_* are CUDA DEVICE pointers owned by
+ *     the caller; pointers named h_* are HOST pointers owned by the caller.
+ *   - `stream` is a cudaStream_t passed as void* (0 = legacy default stream).  Calls
+ *     are asynchronous on `stream` unless the comment says "synchronises".
+ *   - Return value: TKHP_OK (0) or a negative TKHP_E* code; nothing is thrown across
+ *     the ABI.  After an error the contents of output arrays are unspecified and
+ *     tkhp_last_error() describes the failure.
+ *   - No allocation after tkhp_create(): all device memory is the caller's workspace.
+ *   - A context is not thread-safe; use one per host thread / stream.
+ *   - There is no CPU fallback: without a CUDA device tkhp_create() fails (TKHP_ECUDA).
+ */
+#ifndef TKHP_H
+#define TKHP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tkhp_ctx tkhp_ctx; /* opaque; owned by the library */
+
+enum {
+    TKHP_OK = 0,
+    TKHP_EINVAL = -1,     /* bad argument / parameter out of the supported range */
+    TKHP_ECUDA = -2,      /* CUDA runtime error or no device */
+    TKHP_ECUTOFF = -3,    /* cutoff + skin > box/2 (single minimum image only) */
+    TKHP_ENOLIST = -4,    /* tkhp_nblist_build() has not been called on this context */
+    TKHP_ENOCONV = -5,    /* PCG hit max_iter; d_mu holds the best iterate */
+    TKHP_ECAPACITY = -6,  /* workspace too small for this geometry (see max_* params) */
+    TKHP_ENONFINITE = -7  /* NaN/Inf in positions, or polarizability <= 0 */
+};
+
+/* precision of the pair arithmetic (DP and MP modes) */
+enum {
+    TKHP_FP64 = 0,  /* every operation in FP64 */
+    TKHP_MIXED = 1  /* FP32 pair math, FP64 accumulation of fields and of all dot products */
+};
+
+/* which pair-list the compute kernels walk (both are built from the same 32-atom blocks) */
+enum {
+    TKHP_LIST_TILES = 0,   /* one warp per 32x32 block pair of the block-pair list */
+    TKHP_LIST_CLUSTER = 1  /* filtered 8-atom-cluster -> atom lists, the paper's "list filtering"
+                               at finer granularity; falls back to TILES when the
+                              box is too small for it (box/2 < cutoff + block extent) */
+};
+
+typedef struct {
+    int32_t n_atoms;     /* N >= 1 */
+    int32_t precision;   /* TKHP_FP64 | TKHP_MIXED */
+    int32_t device;      /* CUDA device ordinal */
+    int32_t list_mode;   /* TKHP_LIST_TILES | TKHP_LIST_CLUSTER */
+    double box;          /* cubic box edge L; <= 0: open boundary, no images (tests) */
+    double cutoff;       /* r_c: a pair contributes iff R^2 <= r_c^2 */
+    double skin;         /* list buffer: block pairs kept by box distance <= r_c + skin */
+    double ewald_beta;   /* Ewald coefficient beta (1/A); 0: bare Coulomb, no self term (tests) */
+    double thole_a;      /* Thole width a (0.39 for AMOEBA water) */
+    int32_t max_tiles_per_block; /* capacity of the block-pair list per block; 0 = automatic */
+    int32_t max_nbrs_per_cluster; /* capacity of a cluster's atom list; 0 = automatic */
+} tkhp_params;
+
+/* Bytes of device workspace tkhp_create() needs for these parameters.  Host, pure. */
+int tkhp_workspace_bytes(const tkhp_params *params, size_t *bytes);
+
+/* Create a context on params->device using caller-owned device memory d_workspace
+ * (>= tkhp_workspace_bytes, 256-byte aligned).  Synchronises.  *out is NULL on error. */
+int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp_ctx **out);
+int tkhp_destroy(tkhp_ctx *ctx);
+
+/* Text of the last error on this context (ctx-owned, valid until the next call);
+ * with ctx == NULL: the last error of a failed tkhp_create() on this thread. */
+const char *tkhp_last_error(const tkhp_ctx *ctx);
+
+/*
+ * Neighbour list (P:L310-366 cells -> groups of B_size = 32 -> group-pair list;
+ * BASELINE.json north_star: "atoms are sorted spatially into 32-atom blocks, and block
+ * pairs are kept by bounding-box distance against the cutoff plus a skin").
+ *   d_pos            N*3  positions (x,y,z per atom), any image
+ *   d_polarizability N    alpha_i > 0
+ *   d_group_id       N    polarization group, 0 <= g < N (same group => masked pair)
+ * Steps: wrap, Hilbert cell key on a 2^b grid, stable sort by (key, index), gather to
+ * block-local structure-of-arrays, per-block bounding boxes, block pairs (I <= J) with
+ * box gap^2 <= (cutoff+skin)^2 (FP64, no FMA contraction: DESIGN.md section 3), and, in
+ * CLUSTER mode, the filtered cluster->atom lists at r_c.  The positions passed here are
+ * the positions every later call on this context uses.
+ */
+int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polarizability,
+                      const int32_t *d_group_id, void *stream);
+
+/* Read-only view of the list.  Synchronises `stream`.  Pointers stay valid until the
+ * next tkhp_nblist_build()/tkhp_destroy().
+ *   *d_perm   32*n_blocks int32: original atom index per sorted slot, -1 = phantom
+ *             (phantoms only at the end of the last block)
+ *   *d_pairs  2*n_pairs int32: (I,J), I <= J, sorted lexicographically            */
+int tkhp_nblist_view(tkhp_ctx *ctx, int32_t *n_blocks, int64_t *n_pairs,
+                     const int32_t **d_perm, const int32_t **d_pairs, void *stream);
+
+/* Statistics of the current list.  Synchronises `stream`.  Any pointer may be NULL.
+ *   n_pairs_within_cutoff  unordered atom pairs {i,j}, i != j, R^2 <= r_c^2 (FP64 test):
+ *                          the "useful pair interactions" of one field / T.mu evaluation
+ *   n_slots_evaluated      lane-slots the compute kernels of the active list mode walk
+ *                          per evaluation (tiles: 1024 per off-diagonal tile, 992 per
+ *                          diagonal tile; cluster: 8 x list length summed over clusters)
+ *   list_mode_in_use       TKHP_LIST_TILES or TKHP_LIST_CLUSTER after any fallback   */
+int tkhp_nblist_stats(tkhp_ctx *ctx, int64_t *n_pairs_within_cutoff, int64_t *n_slots_evaluated,
+                      int32_t *list_mode_in_use, void *stream);
+
+/*
+ * Permanent-multipole field (F1-F3; charge, dipole, traceless quadrupole,
+ * erfc-damped real-space Ewald with Thole damping; same-group pairs masked; Ewald self
+ * term on d_i).  "Same strategy for the other real space kernels (electrostatics and
+ * polarization)"; masked pairs in a separate FP64 pass.
+ *   d_charge N, d_dipole N*3, d_quad N*6 (xx,xy,xz,yy,yz,zz; traceless Cartesian),
+ *   d_field  N*3 out (e/A^2).
+ */
+int tkhp_perm_field(tkhp_ctx *ctx, const double *d_charge, const double *d_dipole,
+                    const double *d_quad, double *d_field, void *stream);
+
+/* d_out = T_real d_mu + (4 beta^3 / (3 sqrt(pi))) d_mu   (T1-T2; "the matrix-vector
+ * product").  d_mu, d_out: N*3; must not alias. */
+int tkhp_tmatvec(tkhp_ctx *ctx, const double *d_mu, double *d_out, void *stream);
+
+/*
+ * Solve (alpha^-1 - T) mu = field by conjugate gradients with the diagonal (Jacobi)
+ * preconditioner alpha (recurrences in DESIGN.md S).
+ *   d_field   N*3 right-hand side
+ *   d_mu      N*3 in: initial guess if use_guess != 0 (else alpha*field is used); out: mu
+ *   tol       stop when sqrt(sum_i |r_i|^2 / N) < tol  (e/A^2)
+ *   h_iters   host out: number of T.p products in the loop;  h_rms host out: final rms
+ * Synchronises `stream` (convergence is read back by the host).  Returns TKHP_ENOCONV
+ * (with the best mu) when max_iter is reached.
+ */
+int tkhp_polar_solve(tkhp_ctx *ctx, const double *d_field, double *d_mu, double tol,
+                     int32_t max_iter, int32_t use_guess, int32_t *h_iters, double *h_rms,
+                     void *stream);
+
+/* *d_energy (device, 1 double) = -1/2 * 332.063713 * sum_i mu_i . field_i  (kcal/mol). */
+int tkhp_polar_energy(tkhp_ctx *ctx, const double *d_mu, const double *d_field,
+                      double *d_energy, void *stream);
+
+/*
+ * Whole hot path from HOST buffers (end-to-end entry used for the e2e benchmark leg):
+ * copies the inputs to the device, builds the list, evaluates the field, solves for mu,
+ * computes E_pol and copies mu, field and E_pol back.  Host arrays as in the calls above.
+ * The staging buffers come from the context's workspace.  Synchronises.
+ */
+int tkhp_polarize_host(tkhp_ctx *ctx, const double *h_pos, const double *h_polarizability,
+                       const int32_t *h_group_id, const double *h_charge, const double *h_dipole,
+                       const double *h_quad, double tol, int32_t max_iter,
+                       double *h_mu /* N*3 out, may be NULL */,
+                       double *h_field /* N*3 out, may be NULL */, double *h_energy /* 1 out */,
+                       int32_t *h_iters, double *h_rms, void *stream);
+
+/* Timing of the internal phases of the most recent call that ran them, in ms, measured with
+ * CUDA events on the call's stream: [0] list build, [1] field, [2] last T.mu kernel,
+ * [3] solve, [4] energy.  Synchronises the events.  Any entry not run yet is < 0. */
+int tkhp_last_timings(tkhp_ctx *ctx, double ms[5]);
+
+/*
+ * Register-resident FMA microbenchmark used as the measured ALU roofline denominator
+ * (SURVEY 8(d) "Peaks"): runs dependent-chain FMAs with 8 accumulators per thread on every
+ * SM for about `seconds`, returns sustained TFLOP/s (2 flops per FMA).
+ *   precision: TKHP_MIXED -> FP32 FFMA, TKHP_FP64 -> DFMA.   Synchronises.
+ */
+int tkhp_fma_peak(int32_t device, int32_t precision, double seconds, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TKHP_H */

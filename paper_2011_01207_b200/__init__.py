@@ -1,0 +1,27 @@
+"""paper_2011_01207_b200 -- thin Python binding of libtkhp (include/tkhp.h).
+
+Real-space AMOEBA polarization (blocked neighbour list -> permanent field ->
+T.mu / PCG solve -> energy) on one NVIDIA B200, after arXiv 2011.01207.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of
+``csrc/``.  PyTorch supplies device memory and streams, nothing else.  There is
+no CPU fallback: importing works without a GPU (so the build can be checked),
+but creating a context without a CUDA device raises, and a missing
+``libtkhp.so`` raises at import of :mod:`paper_2011_01207_b200.binding`.
+"""
+from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_LIST_TILES, TKHP_LIST_CLUSTER,
+                      TkhpError, TkhpParams, Polarizer, lib, lib_path,
+                      tkhp_workspace_bytes, tkhp_create, tkhp_destroy, tkhp_last_error,
+                      tkhp_nblist_build, tkhp_nblist_view, tkhp_nblist_stats,
+                      tkhp_perm_field, tkhp_tmatvec, tkhp_polar_solve,
+                      tkhp_polar_energy, tkhp_polarize_host, tkhp_last_timings,
+                      tkhp_fma_peak, EXPORTED_SYMBOLS)
+
+__all__ = [
+    "TKHP_FP64", "TKHP_MIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TkhpError",
+    "TkhpParams", "Polarizer", "lib", "lib_path", "tkhp_workspace_bytes", "tkhp_create",
+    "tkhp_destroy", "tkhp_last_error", "tkhp_nblist_build", "tkhp_nblist_view",
+    "tkhp_nblist_stats", "tkhp_perm_field", "tkhp_tmatvec", "tkhp_polar_solve",
+    "tkhp_polar_energy", "tkhp_polarize_host", "tkhp_last_timings", "tkhp_fma_peak",
+    "EXPORTED_SYMBOLS",
+]

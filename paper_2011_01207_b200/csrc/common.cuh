@@ -1,0 +1,179 @@
+// common.cuh -- context, workspace layout and small helpers shared by the .cu files of libtkhp.
+// B200 / sm_100a only.  No code here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/tkhp.h"
+
+namespace tkhp {
+
+constexpr int BLOCK = 32;          // B_size: atoms per block = warp size
+constexpr int CLUSTER = 8;         // atoms per cluster in CLUSTER list mode
+constexpr int SUPER = 32;          // blocks per super-block in the hierarchical pair search
+constexpr int MAX_PARTIALS = 1024; // reduction partials per dot product
+constexpr double COULOMB = 332.063713;          // kcal A / (mol e^2)  (DESIGN.md U)
+constexpr double SQRT_PI = 1.772453850905516027298167483341;
+constexpr float PHANTOM_FAR = 1.0e6f;            // local coordinate of phantom atoms (A)
+
+// Device-resident scalars written by kernels and read by later kernels or by the host.
+struct DeviceState {
+    // error flags (sticky until the next build)
+    int err_nonfinite;      // NaN/Inf position
+    int err_bad_alpha;      // alpha <= 0
+    int err_bad_group;      // group id outside [0, N)
+    int err_capacity;       // tile list or cluster list overflow
+    // grid (sort key)
+    int grid_bits;          // b
+    int pad0;
+    double grid_origin[3];  // 0 when periodic, per-axis minimum when open
+    double grid_inv_h;      // 2^b / extent
+    double lo[3], hi[3];    // open-boundary extent reduction
+    // geometry
+    unsigned long long max_half_bits;   // max block half-extent over all axes (bits of a double >= 0)
+    int per_pair_image;                 // 1: box too small for one image shift per tile
+    int cluster_ok;                     // 1: CLUSTER lists valid for this geometry
+    // list sizes
+    long long n_tiles;                  // block pairs kept
+    long long n_diag_tiles;
+    long long n_cluster_entries;        // total entries of all cluster lists (CLUSTER mode)
+    long long n_pairs_within_cutoff;    // statistics (tkhp_nblist_stats)
+    // PCG scalars
+    double rz, pq, rr, gamma, delta;
+    int converged;
+    int iters;
+};
+
+struct Ctx {
+    tkhp_params p;
+    int n, n_blocks, n_pad, n_super;
+    int sm_count;
+    bool built;
+    int list_mode_in_use;
+    long long cap_tiles;
+    long long n_tiles_host;             // valid after a view/stats/solve sync
+    int n_cells_alloc;                  // 2^(3 b_alloc)
+    int grid_bits_host;                 // periodic: b ; open: -1 (computed on device)
+    char err[512];
+
+    // ---- workspace carve (device pointers) ----
+    DeviceState *st;
+    // sort
+    uint32_t *key;          // N
+    uint32_t *cell_count;   // n_cells_alloc + 1  (also reused for group histogram: needs >= N+1)
+    uint32_t *cell_start;   // n_cells_alloc + 1
+    uint32_t *scan_tmp;     // block sums for the scan
+    int32_t *tmp_idx;       // N
+    int32_t *perm;          // n_pad, -1 = phantom
+    // copies of the caller's build inputs in ORIGINAL order (the list is valid for these positions)
+    double *pos_o;          // 3 N
+    int32_t *group_o;       // N
+    // polarization groups (mask correction)
+    uint32_t *grp_start;    // N + 1
+    int32_t *grp_members;   // N
+    // sorted, block-local structure of arrays
+    float4 *xyzw32;         // n_pad: local x,y,z (A), w = (a/alpha)^(1/6)
+    double4 *xyzw64;        // n_pad (FP64 mode)
+    double4 *bcentre;       // n_blocks: block box centre (x,y,z, 0)
+    double4 *bhalf;         // n_blocks: half extent
+    double4 *scentre, *shalf; // n_super: super-block boxes
+    double *alpha_s;        // n_pad (0 for phantoms)
+    double *inv_alpha_s;    // n_pad (0 for phantoms)
+    // block-pair list
+    uint32_t *row_count;    // n_blocks + 1
+    uint32_t *row_start;    // n_blocks + 1
+    int2 *pairs;            // cap_tiles
+    // per-evaluation data
+    double *acc;            // 3 * n_pad (SoA x|y|z), FP64 accumulators
+    float4 *mu32;           // n_pad
+    double4 *mu64;          // n_pad
+    float4 *mp32;           // 3 * n_pad: (q,dx,dy,dz) (Qxx,Qxy,Qxz,Qyy) (Qyz,Qzz,group,0)
+    double4 *mp64;          // 3 * n_pad
+    // PCG vectors, sorted order, SoA 3 * n_pad each
+    double *vE, *vmu, *vr, *vp, *vq;
+    double *partials;       // 4 sets (rz ping, rz pong, pq, energy) of 2 * MAX_PARTIALS
+    double *h_scalars;      // pinned host scratch (8 doubles) for scalar read-backs
+    DeviceState *h_state;   // pinned host copy of *st (list header), valid when header_valid
+    bool header_valid;
+    // host-entry staging (tkhp_polarize_host)
+    double *h_pos, *h_alpha, *h_charge, *h_dipole, *h_quad, *h_field, *h_mu, *h_energy;
+    int32_t *h_group;
+    // CLUSTER mode lists (see cluster.cu)
+    void *cl_ws;
+    size_t cl_ws_bytes;
+
+    cudaEvent_t ev[10];
+    double last_ms[5];
+};
+
+// Bump allocator over the caller's workspace; with base == nullptr it only measures.
+struct Carver {
+    char *base;
+    size_t off = 0;
+    explicit Carver(void *b) : base(static_cast<char *>(b)) {}
+    template <typename T>
+    T *take(size_t count) {
+        off = (off + 255) & ~size_t(255);
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+
+inline int set_err(Ctx *c, int code, const char *fmt, const char *a = "") {
+    if (c) snprintf(c->err, sizeof(c->err), fmt, a);
+    return code;
+}
+
+#define TKHP_CUDA(ctx, call)                                                          \
+    do {                                                                              \
+        cudaError_t e_ = (call);                                                      \
+        if (e_ != cudaSuccess) {                                                      \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, \
+                     cudaGetErrorString(e_));                                         \
+            return TKHP_ECUDA;                                                        \
+        }                                                                             \
+    } while (0)
+
+inline int div_up(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// ---- host-side launchers implemented in the other translation units ----
+int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32_t *d_group,
+                 cudaStream_t s);
+int nblist_count_pairs(Ctx *c, cudaStream_t s);
+int tiles_tmatvec(Ctx *c, cudaStream_t s);          // acc = T_real * (mu32|mu64), sorted space
+int tiles_field(Ctx *c, cudaStream_t s);            // acc = unmasked inter-group field
+size_t cluster_workspace_bytes(const tkhp_params *p, int n_blocks);
+int cluster_build(Ctx *c, cudaStream_t s);
+int cluster_tmatvec(Ctx *c, cudaStream_t s);
+int cluster_field(Ctx *c, cudaStream_t s);
+long long cluster_slots(Ctx *c);
+
+int run_tmatvec(Ctx *c, cudaStream_t s);            // dispatch on list mode; zeroes acc first
+int run_field(Ctx *c, cudaStream_t s);
+int do_perm_field(Ctx *c, const double *d_q, const double *d_dip, const double *d_quad, double *d_field,
+                  cudaStream_t s);
+int do_tmatvec(Ctx *c, const double *d_mu, double *d_out, cudaStream_t s);
+int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int max_iter, int use_guess,
+                   int *h_iters, double *h_rms, cudaStream_t s);
+int do_polar_energy(Ctx *c, const double *d_mu, const double *d_field, double *d_energy, cudaStream_t s);
+int ensure_header(Ctx *c, cudaStream_t s);          // list header on the host (one small sync per build)
+
+// warp helpers
+__device__ __forceinline__ double warp_min(double v) {
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+}  // namespace tkhp

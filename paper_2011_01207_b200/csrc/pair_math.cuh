@@ -1,0 +1,180 @@
+// pair_math.cuh -- per-pair arithmetic of the real-space AMOEBA polarization kernels.
+//
+// The paper prints no interaction formula (refs only); these functions
+// implement DESIGN.md section 2 (= SURVEY 8(c)):
+//   Ewald   bn_0 = erfc(bR)/R,  bn_k = [(2k-1) bn_{k-1} + (2b^2)^k/(b sqrt(pi)) exp(-b^2R^2)]/R^2
+//   Thole   x = a R^3/sqrt(alpha_i alpha_j) = (R w_i w_j)^3, w = (a/alpha)^(1/6)
+//           1-lam3 = e^-x, 1-lam5 = (1+x)e^-x, 1-lam7 = (1+x+0.6x^2)e^-x
+//   (F1)    G_k = bn_k - (1 - lam_{2k+1}) rr_k        (unmasked pairs; masked pairs: correction pass)
+//   (F2)    E_i += [q_j G1 + G2 (d_j.R) + (G3/3)(R.Q_j R)] R - G1 d_j - (2/3) G2 (Q_j R)
+//   (T1,T2) m1 = G1, m2 = G2 ;  (T mu)_i += -m1 mu_j + m2 (mu_j.R) R
+// with R = r_i - r_j.  Written so that R^(2k+1) G_k is formed first (one common e^{-z^2} factor),
+// then scaled by R^-(2k+1):  R^3 bn1 = e^{-z^2}[erfcx(z) + c z],  R^5 bn2 = e^{-z^2}[3(..) + 2c z^3],
+// R^7 bn3 = e^{-z^2}[15(..) + 10 c z^3 + 4 c z^5],  z = bR, c = 2/sqrt(pi).
+//
+// MIXED (float): erfcx by the degree-8 polynomial of erfcx_coeffs.h in u = 1/(1+0.4z)
+// (MUFU.RCP), exponentials by ex2.approx, 1/R by MUFU.RSQ: 4 MUFU + ~45 FMA-pipe ops per pair.
+// FP64 (double): erfc()/exp() of the CUDA math library.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include "erfcx_coeffs.h"
+
+namespace tkhp {
+
+template <typename real>
+struct PairConsts {
+    real beta;      // Ewald coefficient
+    real c1;        // 2/sqrt(pi) (0 when beta == 0 in FP64 mode: no exp term)
+    real rc2;       // cutoff^2
+    real box;       // box edge (PPI kernels)
+    real inv_box;
+};
+
+template <typename real> struct Vec4;
+template <> struct Vec4<float> { using type = float4; };
+template <> struct Vec4<double> { using type = double4; };
+
+__device__ __forceinline__ float fast_rcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float fast_ex2(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float fast_rsqrt(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// erfc(z) exp(z^2), 0 <= z <= 6, relative error ~4e-7 in FP32
+__device__ __forceinline__ float erfcx_f32(float z) {
+    constexpr float c[TKHP_ERFCX_DEG + 1] = TKHP_ERFCX_COEFFS;
+    const float u = fast_rcp(fmaf(TKHP_ERFCX_P, z, 1.0f));
+    float p = c[TKHP_ERFCX_DEG];
+#pragma unroll
+    for (int k = TKHP_ERFCX_DEG - 1; k >= 0; --k) p = fmaf(p, u, c[k]);
+    return p;
+}
+
+// ---- MIXED: G_1..G_NK for an unmasked pair -------------------------------------------------
+template <int NK>
+__device__ __forceinline__ void radial_f32(float r2, float ww, const PairConsts<float> &k, float *G) {
+    const float rinv = fast_rsqrt(r2);
+    const float r = r2 * rinv;
+    const float rinv2 = rinv * rinv;
+    const float z = k.beta * r;
+    const float z2 = z * z;
+    const float ez = fast_ex2(z2 * -1.4426950408889634f);
+    const float g1 = fmaf(k.c1, z, erfcx_f32(z));      // erfcx(z) + c z
+    const float t = r * ww;
+    const float x = t * t * t;
+    const float et = fast_ex2(x * -1.4426950408889634f);
+    const float rinv3 = rinv2 * rinv;
+    G[0] = fmaf(ez, g1, -et) * rinv3;
+    if (NK >= 2) {
+        const float cz3 = k.c1 * z * z2;               // c z^3
+        const float h2 = fmaf(2.0f, cz3, 3.0f * g1);   // 3 g1 + 2 c z^3
+        const float rinv5 = rinv3 * rinv2;
+        const float d5 = 3.0f * fmaf(x, et, et);       // 3 (1+x) e^-x
+        G[1] = fmaf(ez, h2, -d5) * rinv5;
+        if (NK >= 3) {
+            const float h3 = fmaf(4.0f * cz3, z2, 5.0f * h2);            // 5 h2 + 4 c z^5
+            const float d7 = 15.0f * fmaf(fmaf(0.6f, x, 1.0f) * x, et, et);  // 15 (1+x+0.6x^2) e^-x
+            G[2] = fmaf(ez, h3, -d7) * (rinv5 * rinv2);
+        }
+    }
+}
+
+// ---- FP64: G_1..G_NK for an unmasked pair --------------------------------------------------
+template <int NK>
+__device__ __forceinline__ void radial_f64(double r2, double ww, const PairConsts<double> &k, double *G) {
+    const double r = sqrt(r2);
+    const double rinv = 1.0 / r;
+    const double rinv2 = rinv * rinv;
+    const double z = k.beta * r;
+    const double ez = exp(-z * z);
+    // R^(2k+1) bn_k by the upward recursion, written in z:  B1 = erfc(z) + c z ez
+    const double cz = k.c1 * z;
+    const double z2 = z * z;
+    const double B1 = erfc(z) + cz * ez;
+    const double t = r * ww;
+    const double x = t * t * t;
+    const double et = exp(-x);
+    const double rinv3 = rinv2 * rinv;
+    G[0] = (B1 - et) * rinv3;
+    if (NK >= 2) {
+        const double B2 = 3.0 * B1 + 2.0 * cz * z2 * ez;
+        const double rinv5 = rinv3 * rinv2;
+        G[1] = (B2 - 3.0 * (1.0 + x) * et) * rinv5;
+        if (NK >= 3) {
+            const double B3 = 5.0 * B2 + 4.0 * cz * z2 * z2 * ez;
+            G[2] = (B3 - 15.0 * (1.0 + x + 0.6 * x * x) * et) * (rinv5 * rinv2);
+        }
+    }
+}
+
+template <int NK>
+__device__ __forceinline__ void radial(float r2, float ww, const PairConsts<float> &k, float *G) {
+    radial_f32<NK>(r2, ww, k, G);
+}
+template <int NK>
+__device__ __forceinline__ void radial(double r2, double ww, const PairConsts<double> &k, double *G) {
+    radial_f64<NK>(r2, ww, k, G);
+}
+
+// ---- masked pair (same polarization group), FP64 only: G_k = bn_k - rr_k --------------------
+// Cancellation-prone (10x..1400x at R ~ 1 A, SURVEY hard part 3): always evaluated in FP64 in the
+// correction pass ("correct_scaling" second kernel of the paper).
+__device__ __forceinline__ void radial_masked_f64(double r2, double beta, double *G) {
+    const double r = sqrt(r2);
+    const double rinv = 1.0 / r;
+    const double rinv2 = rinv * rinv;
+    const double z = beta * r;
+    const double z2 = z * z;
+    const double ez = exp(-z2);
+    const double cz = (beta > 0.0 ? 1.1283791670955125739 : 0.0) * z;   // 2/sqrt(pi) z
+    // B_k - (2k-1)!! with erfc(z) - 1 = -erf(z): no cancellation against the bare Coulomb term
+    const double B1m = -erf(z) + cz * ez;
+    const double B2m = 3.0 * B1m + 2.0 * cz * z2 * ez;
+    const double B3m = 5.0 * B2m + 4.0 * cz * z2 * z2 * ez;
+    const double rinv3 = rinv2 * rinv, rinv5 = rinv3 * rinv2;
+    G[0] = B1m * rinv3;
+    G[1] = B2m * rinv5;
+    G[2] = B3m * rinv5 * rinv2;
+}
+
+// ---- (T1,T2) one direction: out += -m1 mu + m2 (mu.R) R ------------------------------------
+template <typename real>
+__device__ __forceinline__ void tmu_apply(real m1, real m2, real Rx, real Ry, real Rz, real mx, real my,
+                                          real mz, real &ox, real &oy, real &oz) {
+    const real c = m2 * (mx * Rx + my * Ry + mz * Rz);
+    ox += c * Rx - m1 * mx;
+    oy += c * Ry - m1 * my;
+    oz += c * Rz - m1 * mz;
+}
+
+// ---- (F2) field at the point R away from a multipole (q, d, Q); sign = +1: R = r_i - r_j ----
+// For the mirrored direction (field at j from i's multipoles) pass (-Rx,-Ry,-Rz).
+template <typename real>
+__device__ __forceinline__ void field_apply(const real *G, real Rx, real Ry, real Rz, real q, real dx, real dy,
+                                            real dz, real qxx, real qxy, real qxz, real qyy, real qyz,
+                                            real qzz, real &ex, real &ey, real &ez) {
+    const real dR = dx * Rx + dy * Ry + dz * Rz;
+    const real tx = qxx * Rx + qxy * Ry + qxz * Rz;
+    const real ty = qxy * Rx + qyy * Ry + qyz * Rz;
+    const real tz = qxz * Rx + qyz * Ry + qzz * Rz;
+    const real RTR = Rx * tx + Ry * ty + Rz * tz;
+    const real rad = q * G[0] + G[1] * dR + (G[2] * (real)(1.0 / 3.0)) * RTR;
+    const real g23 = G[1] * (real)(2.0 / 3.0);
+    ex += rad * Rx - G[0] * dx - g23 * tx;
+    ey += rad * Ry - G[0] * dy - g23 * ty;
+    ez += rad * Rz - G[0] * dz - g23 * tz;
+}
+
+}  // namespace tkhp

@@ -1,0 +1,223 @@
+"""GPU parity: the CUDA library (through the C ABI binding) against the FP64 CPU oracle,
+element by element on the same seeded inputs.  Tolerances are BASELINE.json's:
+pair set bit-exact; field and T.mu rel-L2 <= 1e-5 (MIXED) / 1e-11 (FP64);
+induced dipoles <= 1e-5 relative; energy <= 1e-6 relative."""
+import numpy as np
+import pytest
+
+import oracle
+from synth_inputs import make_config, tiny_cluster, water_box
+
+pytestmark = pytest.mark.gpu
+
+TOL_VEC = {"fp64": 1e-11, "mixed": 1e-5}
+
+
+def _pk():
+    import paper_2011_01207_b200 as pk
+    return pk
+
+
+def _rel_l2(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b))
+
+
+def _polarizer(s, precision, list_mode="tiles"):
+    pk = _pk()
+    P = pk.Polarizer.for_system(
+        s, precision=pk.TKHP_FP64 if precision == "fp64" else pk.TKHP_MIXED,
+        list_mode=pk.TKHP_LIST_TILES if list_mode == "tiles" else pk.TKHP_LIST_CLUSTER)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    return P
+
+
+SYSTEMS = {
+    "cfg0": lambda: make_config(0),
+    "n2_open": lambda: tiny_cluster(2, 1, box=0.0, spread=2.0, group_size=1),
+    "n3_open_onegroup": lambda: tiny_cluster(3, 2, box=0.0, spread=2.5, group_size=3),
+    "n33_open": lambda: tiny_cluster(33, 3, box=0.0, spread=7.0, cutoff=5.0),
+    "n65_periodic": lambda: tiny_cluster(65, 4, box=14.0, spread=14.0, cutoff=5.0, skin=1.0, ewald_beta=0.6),
+    "n200_periodic_noewald": lambda: tiny_cluster(200, 5, box=20.0, spread=20.0, cutoff=6.0, skin=1.0),
+    "water_1536_solutes": lambda: water_box(512, 24.85, 77, solute_frac=0.15),
+}
+
+
+@pytest.fixture(scope="module", params=list(SYSTEMS))
+def system(request):
+    return SYSTEMS[request.param]()
+
+
+# ------------------------------------------------------------------ neighbour list
+def test_nblist_pair_set_is_bit_exact(system):
+    s = system
+    P = _polarizer(s, "mixed")
+    perm, pairs = P.nblist_view()
+    oracle.check_perm(perm, s.pos, s.box)                       # (N i, ii)
+    want = oracle.block_pairs(perm, s.pos, s.box, s.cutoff + s.skin)   # (N iii)
+    order = np.lexsort((pairs[:, 1], pairs[:, 0]))              # canonical sort
+    assert np.array_equal(pairs[order], want)
+    assert np.array_equal(order, np.arange(len(order))), "library list must already be sorted"
+    n_pair, n_slots, mode = P.nblist_stats()
+    assert n_pair == oracle.count_pairs(s)
+    if s.n_atoms <= 2000:
+        assert oracle.atom_pairs_covered(perm, pairs, s.pos, s.box, s.cutoff + s.skin)   # (N iv)
+    P.close()
+
+
+def test_nblist_is_deterministic_and_rebuildable():
+    s = make_config(0)
+    P = _polarizer(s, "mixed")
+    perm1, pairs1 = P.nblist_view()
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    perm2, pairs2 = P.nblist_view()
+    assert np.array_equal(perm1, perm2) and np.array_equal(pairs1, pairs2)
+    # moved atoms -> different list on the same context
+    P.nblist_build(s.pos + 0.37, s.polarizability, s.group_id)
+    perm3, pairs3 = P.nblist_view()
+    oracle.check_perm(perm3, s.pos + 0.37, s.box)
+    assert np.array_equal(pairs3, oracle.block_pairs(perm3, s.pos + 0.37, s.box, s.cutoff + s.skin))
+    P.close()
+
+
+# ------------------------------------------------------------------ T.mu and field
+@pytest.mark.parametrize("precision", ["fp64", "mixed"])
+def test_tmatvec_matches_oracle(system, precision):
+    s = system
+    rng = np.random.default_rng(42)
+    mu = rng.standard_normal((s.n_atoms, 3)) * 0.1
+    want = oracle.tmatvec(s, mu)
+    P = _polarizer(s, precision)
+    got = P.tmatvec(mu).cpu().numpy()
+    assert _rel_l2(got, want) <= TOL_VEC[precision]
+    P.close()
+
+
+@pytest.mark.parametrize("precision", ["fp64", "mixed"])
+def test_perm_field_matches_oracle(system, precision):
+    s = system
+    want = oracle.perm_field(s)
+    P = _polarizer(s, precision)
+    got = P.perm_field(s.charge, s.dipole, s.quad).cpu().numpy()
+    if np.linalg.norm(want) == 0.0:
+        assert np.abs(got).max() < 1e-12
+    else:
+        assert _rel_l2(got, want) <= TOL_VEC[precision]
+    P.close()
+
+
+def test_tmatvec_symmetry_on_gpu():
+    """nu.T mu == mu.T nu for the GPU operator as well (FP64 mode)."""
+    import torch
+    s = make_config(0)
+    P = _polarizer(s, "fp64")
+    rng = np.random.default_rng(9)
+    mu, nu = rng.standard_normal((2, s.n_atoms, 3))
+    a = float((torch.as_tensor(nu, device="cuda") * P.tmatvec(mu)).sum())
+    b = float((torch.as_tensor(mu, device="cuda") * P.tmatvec(nu)).sum())
+    assert abs(a - b) <= 1e-12 * max(abs(a), abs(b))
+    P.close()
+
+
+# ------------------------------------------------------------------ solve and energy
+@pytest.mark.parametrize("precision", ["fp64", "mixed"])
+@pytest.mark.parametrize("name", ["cfg0", "n65_periodic", "water_1536_solutes"])
+def test_solve_and_energy_match_oracle(name, precision):
+    """Q11: both sides converge tighter than the parity bar so that truncation error does not
+    mask arithmetic error (oracle: dense Cholesky; GPU: 1e-12 FP64 / 1e-8 MIXED)."""
+    s = SYSTEMS[name]()
+    E = oracle.perm_field(s)
+    mu_ref = oracle.dense_solve(s, E)
+    e_ref = oracle.polar_energy(mu_ref, E)
+    P = _polarizer(s, precision)
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    tol = 1e-12 if precision == "fp64" else 1e-8
+    mu, it, rms = P.polar_solve(Eg, tol=tol, max_iter=100)
+    assert rms < tol and 0 < it < 40
+    mu_h = mu.cpu().numpy()
+    assert _rel_l2(mu_h, mu_ref) <= (1e-10 if precision == "fp64" else 1e-5)
+    e_gpu = float(P.polar_energy(mu, Eg).cpu())
+    assert abs(e_gpu - e_ref) <= (1e-10 if precision == "fp64" else 1e-6) * abs(e_ref)
+    P.close()
+
+
+def test_solve_iteration_counts_and_guess():
+    s = make_config(0)
+    P = _polarizer(s, "fp64")
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    E = Eg.cpu().numpy()
+    for tol in (1e-5, 1e-6, 1e-8):
+        _, it_ref, _ = oracle.pcg_solve(s, E, tol=tol)
+        mu, it, rms = P.polar_solve(Eg, tol=tol)
+        assert it == it_ref and rms < tol
+    mu2, it2, rms2 = P.polar_solve(Eg, tol=1e-8, guess=mu)
+    assert it2 == 0
+    pk = _pk()
+    with pytest.raises(pk.TkhpError) as e:
+        P.polar_solve(Eg, tol=1e-30, max_iter=2)
+    assert e.value.code == -5
+    P.close()
+
+
+def test_two_site_closed_form_through_the_library(golden):
+    """Pin P8 through the GPU path (open boundary, beta = 0)."""
+    import torch
+    from synth_inputs import System
+    g = golden["P8_two_site"]
+    s = System(name="two", box=0.0, pos=np.array([[0, 0, 0], [0, 0, g["R"]]], float),
+               charge=np.zeros(2), dipole=np.zeros((2, 3)), quad=np.zeros((2, 6)),
+               polarizability=np.array(g["alpha"]), group_id=np.array([0, 1], np.int32),
+               cutoff=7.0, skin=2.0, ewald_beta=0.0, thole_a=g["a"])
+    P = _polarizer(s, "fp64")
+    for axis, key in ((2, "par"), (0, "perp")):
+        E = np.zeros((2, 3)); E[:, axis] = g["E"]
+        mu, it, rms = P.polar_solve(E, tol=1e-14)
+        np.testing.assert_allclose(mu.cpu().numpy()[:, axis], g["mu_" + key], rtol=1e-12)
+        e = float(P.polar_energy(mu, torch.as_tensor(E, device="cuda")).cpu())
+        assert e == pytest.approx(g["Epol_" + key], rel=1e-12)
+    P.close()
+
+
+# ------------------------------------------------------------------ host entry and errors
+def test_polarize_host_matches_device_calls():
+    pk = _pk()
+    s = make_config(0)
+    P = _polarizer(s, "mixed")
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    mu, it, rms = P.polar_solve(Eg, tol=1e-6)
+    e = float(P.polar_energy(mu, Eg).cpu())
+    h_mu = np.zeros((s.n_atoms, 3)); h_E = np.zeros((s.n_atoms, 3)); h_e = np.zeros(1)
+    it2, rms2, ok = pk.tkhp_polarize_host(P.ctx, s.pos, s.polarizability, s.group_id, s.charge,
+                                          s.dipole, s.quad, 1e-6, 100, h_mu, h_E, h_e)
+    assert ok and it2 == it
+    np.testing.assert_allclose(h_E, Eg.cpu().numpy(), rtol=0, atol=1e-9)
+    assert _rel_l2(h_mu, mu.cpu().numpy()) < 1e-6
+    assert abs(h_e[0] - e) < 1e-6 * abs(e)
+    P.close()
+
+
+def test_error_paths_on_device():
+    pk = _pk()
+    s = make_config(0)
+    P = pk.Polarizer.for_system(s)
+    with pytest.raises(pk.TkhpError) as e:
+        P.tmatvec(np.zeros((s.n_atoms, 3)))
+    assert e.value.code == -4                       # TKHP_ENOLIST
+    bad = s.pos.copy(); bad[5, 1] = np.nan
+    P.nblist_build(bad, s.polarizability, s.group_id)
+    with pytest.raises(pk.TkhpError) as e:
+        P.nblist_view()
+    assert e.value.code == -7                       # TKHP_ENONFINITE
+    al = s.polarizability.copy(); al[7] = 0.0
+    P.nblist_build(s.pos, al, s.group_id)
+    with pytest.raises(pk.TkhpError) as e:
+        P.tmatvec(np.zeros((s.n_atoms, 3)))
+    assert e.value.code == -7
+    P.nblist_build(s.pos, s.polarizability, s.group_id)   # context recovers
+    P.tmatvec(np.ones((s.n_atoms, 3)))
+    P.close()
+    tiny = pk.Polarizer.for_system(s, max_tiles_per_block=1)
+    tiny.nblist_build(s.pos, s.polarizability, s.group_id)
+    with pytest.raises(pk.TkhpError) as e:
+        tiny.nblist_view()
+    assert e.value.code == -6                       # TKHP_ECAPACITY
+    tiny.close()
