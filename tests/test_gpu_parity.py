@@ -98,7 +98,7 @@ def test_perm_field_matches_oracle(system, precision):
     want = oracle.perm_field(s)
     P = _polarizer(s, precision)
     got = P.perm_field(s.charge, s.dipole, s.quad).cpu().numpy()
-    if np.linalg.norm(want) == 0.0:
+    if np.linalg.norm(want) < 1e-12:      # isolated masked molecule: field is zero up to rounding
         assert np.abs(got).max() < 1e-12
     else:
         assert _rel_l2(got, want) <= TOL_VEC[precision]
