@@ -1,0 +1,378 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the real-space AMOEBA polarization hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 0|1|2|3] [--precision mixed|fp64] [--list-mode auto|tiles|cluster]
+
+One STEP = one pass of the whole hot path over one synthetic system:
+neighbour-list build -> permanent field -> PCG solve to RMS 1e-6 -> polarization energy
+(BASELINE.json configs[1] wording), by default on the 98,304-atom heterogeneous box
+(configs[2], the system BASELINE.json's target is quoted on) in MIXED precision.
+
+metric/unit: useful pair interactions per second.  One pair interaction = one unordered atom
+pair {i,j} with R <= r_c evaluated once, for both atoms, in the field or in one T.mu product.
+A step performs N_pair * (1 + n_matvec) of them (n_matvec = PCG iterations + 1 for the initial
+residual); value = that / step time, summed over GPUs (replicas: SURVEY 8(e) "replicas only").
+
+Prints ONE JSON line on rank 0 (see DESIGN.md section 8 for every key).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "useful pair interactions/s (field + T.mu matvecs of one list-build + field + PCG solve + energy step)"
+UNIT = "pair interactions/s"
+FLOPS_PER_PAIR_TMU = 89      # 32 FFMA*2 + 22 FMUL + 3 FADD per evaluated slot
+FLOPS_PER_PAIR_FIELD = 160
+# ALU roofline denominator derived in DESIGN.md section 7: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
+PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+PEAK_FP64_TFLOPS = PEAK_FP32_TFLOPS / 2
+WORKLOADS = {0: "cfg0_water648", 1: "cfg1_dhfr_size_23559", 2: "cfg2_hetero_98304", 3: "cfg3_stmv_size_1066629"}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3])
+    ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
+    ap.add_argument("--list-mode", default="auto", choices=["auto", "tiles", "cluster"])
+    ap.add_argument("--tol", type=float, default=1e-6)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--peak-seconds", type=float, default=1.0)
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.lines: list[str] = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._pump, daemon=True)
+        self.thread.start()
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 9:
+                continue
+            try:
+                sm.append(float(parts[1])); smax.append(float(parts[2])); power.append(float(parts[3]))
+            except ValueError:
+                continue
+            for name, flag in zip(names, parts[5:9]):
+                if flag.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(smax), "samples": len(sm),
+                "power_w_max": max(power), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------- CPU oracle legs
+def oracle_sample(sys_, n_rows: int, seed: int = 7):
+    """Time the oracle as it stands on a bounded sample of rows: field + one T.mu on n_rows rows."""
+    import oracle
+    rng = np.random.default_rng(seed)
+    rows = np.sort(rng.choice(sys_.n_atoms, size=min(n_rows, sys_.n_atoms), replace=False)).astype(np.int64)
+    mu = rng.standard_normal((sys_.n_atoms, 3)) * 0.1
+    ordered = oracle.count_pairs_rows(sys_, rows)          # not timed: the unit count
+    t0 = time.perf_counter()
+    oracle.perm_field_rows(sys_, rows)
+    oracle.tmatvec_rows(sys_, mu, rows)
+    dt = time.perf_counter() - t0
+    # ordered evaluations / 2 = unordered-pair equivalents, times 2 operators
+    return {"pair_interactions": float(ordered), "seconds": dt, "rows": int(rows.size),
+            "cores": oracle.num_threads()}
+
+
+def run_reference(args, rank: int, world: int):
+    """--impl reference: the CPU oracle, as it stands, on this arm's config/metric (rank 0 only)."""
+    if rank != 0:
+        return
+    from synth_inputs import make_config
+    import oracle
+    oracle.build()
+    sys_ = make_config(args.config)
+    n_rows = 2048 if sys_.n_atoms > 5000 else sys_.n_atoms
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(sys_, max(64, n_rows // 8))
+    tot_pairs, tot_s = 0.0, 0.0
+    cores = 1
+    for k in range(args.steps):
+        r = oracle_sample(sys_, n_rows, seed=100 + k)
+        tot_pairs += r["pair_interactions"]; tot_s += r["seconds"]; cores = r["cores"]
+    value = tot_pairs / tot_s
+    sample = (f"each step: oracle perm_field + one tmatvec on {n_rows} seeded random rows of "
+              f"{WORKLOADS[args.config]} (O(N) minimum-image loop per row, FP64)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "n_atoms": sys_.n_atoms, "cutoff": sys_.cutoff,
+                   "ewald_beta": sys_.ewald_beta, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- our arm
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import torch
+    import paper_2011_01207_b200 as pk
+    from synth_inputs import make_config
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libtkhp has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=dev)
+        dist = dist_mod
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sys_ = make_config(args.config)
+    n = sys_.n_atoms
+    precision = pk.TKHP_MIXED if args.precision == "mixed" else pk.TKHP_FP64
+    want_mode = {"auto": pk.TKHP_LIST_CLUSTER, "cluster": pk.TKHP_LIST_CLUSTER,
+                 "tiles": pk.TKHP_LIST_TILES}[args.list_mode]
+    P = pk.Polarizer.for_system(sys_, precision=precision, list_mode=want_mode, device=local_rank)
+    f64 = torch.float64
+    d_pos = torch.as_tensor(sys_.pos, dtype=f64, device=dev)
+    d_alpha = torch.as_tensor(sys_.polarizability, dtype=f64, device=dev)
+    d_group = torch.as_tensor(sys_.group_id, dtype=torch.int32, device=dev)
+    d_q = torch.as_tensor(sys_.charge, dtype=f64, device=dev)
+    d_dip = torch.as_tensor(sys_.dipole, dtype=f64, device=dev)
+    d_quad = torch.as_tensor(sys_.quad, dtype=f64, device=dev)
+    d_field = torch.empty((n, 3), dtype=f64, device=dev)
+    d_mu = torch.empty((n, 3), dtype=f64, device=dev)
+    d_energy = torch.empty((), dtype=f64, device=dev)
+    stream = torch.cuda.current_stream()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def step():
+        pk.tkhp_nblist_build(P.ctx, d_pos, d_alpha, d_group, stream)
+        pk.tkhp_perm_field(P.ctx, d_q, d_dip, d_quad, d_field, stream)
+        it, rms, ok = pk.tkhp_polar_solve(P.ctx, d_field, d_mu, args.tol, 100, False, stream)
+        pk.tkhp_polar_energy(P.ctx, d_mu, d_field, d_energy, stream)
+        return it, rms
+
+    for _ in range(max(args.warmup, 3)):
+        it, rms = step()
+    torch.cuda.synchronize()
+    n_pair, n_slots, mode_in_use = P.nblist_stats()
+    energy = float(d_energy.cpu())
+
+    # ---- timed region: K steps, device-resident inputs, L2 flushed between steps
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    pk.tkhp_profile_reset(P.ctx, True)
+    prof_tot = dict(launches=0, n_tmatvec=0, tmatvec_ms=0.0, n_field=0, field_ms=0.0)
+    iters = []
+    sampler.start()
+    barrier()
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.fill_(k & 0xFF)
+        ev[k][0].record(stream)
+        it, rms = step()
+        ev[k][1].record(stream)
+        iters.append(it)
+        pr = pk.tkhp_profile_read(P.ctx)
+        for key in prof_tot:
+            prof_tot[key] += pr[key]
+        pk.tkhp_profile_reset(P.ctx, True)
+    barrier()
+    wall_s = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    phase_ms = P.timings()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
+    if dist is not None:
+        t = torch.tensor([total_ms, wall_s], dtype=f64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, wall_s = float(t[0]), float(t[1])
+    ms_per_step = total_ms / args.steps
+    n_matvec = statistics.mean(iters) + 1
+    pairs_per_step = n_pair * (1 + n_matvec)
+    value = world * pairs_per_step / (ms_per_step * 1e-3)
+
+    # ---- dominant kernel roofline (T.mu pair kernel), measured live with CUDA events
+    tmu_ms = prof_tot["tmatvec_ms"] / max(prof_tot["n_tmatvec"], 1)
+    fld_ms = prof_tot["field_ms"] / max(prof_tot["n_field"], 1)
+    peak = PEAK_FP32_TFLOPS if args.precision == "mixed" else PEAK_FP64_TFLOPS
+    achieved = FLOPS_PER_PAIR_TMU * n_pair / (tmu_ms * 1e-3) / 1e12
+    executed = FLOPS_PER_PAIR_TMU * n_slots / (tmu_ms * 1e-3) / 1e12
+    roofline = {
+        "bound": "alu", "kernel": "T.mu pair kernel (%s list)" % ("cluster" if mode_in_use == pk.TKHP_LIST_CLUSTER else "tiles"),
+        "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+        "traffic": None,
+        "algorithmic_flops_per_launch": FLOPS_PER_PAIR_TMU * n_pair,
+        "avg_launch_ms": tmu_ms, "launches_timed": prof_tot["n_tmatvec"],
+        "share_of_step": prof_tot["tmatvec_ms"] / total_ms if world == 1 else None,
+        "executed_slots_per_launch": n_slots, "executed_tflops_nominal": executed,
+        "executed_frac_of_peak": executed / peak,
+        "useful_pairs_per_s_kernel": n_pair / (tmu_ms * 1e-3),
+        "field_kernel_avg_ms": fld_ms,
+        "peak_note": "148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md section 7)",
+    }
+    try:
+        traffic_file = ROOT / "profiles" / "traffic.json"
+        if traffic_file.exists():
+            roofline["traffic"] = json.loads(traffic_file.read_text()).get(
+                "cluster" if mode_in_use == pk.TKHP_LIST_CLUSTER else "tiles")
+    except Exception:
+        pass
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a, dt: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).pin_memory()
+        h_pos, h_alpha = pin(sys_.pos, f64), pin(sys_.polarizability, f64)
+        h_group = pin(sys_.group_id, torch.int32)
+        h_q, h_dip, h_quad = pin(sys_.charge, f64), pin(sys_.dipole, f64), pin(sys_.quad, f64)
+        h_mu = torch.empty((n, 3), dtype=f64).pin_memory()
+        h_e = torch.empty(1, dtype=f64).pin_memory()
+        for _ in range(2):
+            pk.tkhp_polarize_host(P.ctx, h_pos, h_alpha, h_group, h_q, h_dip, h_quad, args.tol, 100,
+                                  h_mu, None, h_e, stream)
+        barrier()
+        e2e_ms, e2e_iters = [], []
+        for k in range(args.steps):
+            flush.fill_(k & 0xFF)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            it2, _, _ = pk.tkhp_polarize_host(P.ctx, h_pos, h_alpha, h_group, h_q, h_dip, h_quad,
+                                              args.tol, 100, h_mu, None, h_e, stream)
+            _ = float(h_e[0])
+            e2e_ms.append((time.perf_counter() - t0) * 1e3)
+            e2e_iters.append(it2)
+        barrier()
+        tot = sum(e2e_ms)
+        if dist is not None:
+            t = torch.tensor([tot], dtype=f64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            tot = float(t[0])
+        e2e_step = tot / args.steps
+        e2e = {"value": world * n_pair * (2 + statistics.mean(e2e_iters)) / (e2e_step * 1e-3), "unit": UNIT,
+               "ms_per_step": e2e_step,
+               "h2d_bytes_per_step": n * (24 + 8 + 4 + 8 + 24 + 48),
+               "d2h_bytes_per_step": n * 24 + 8}
+
+    # ---- measured FMA peak and the CPU oracle beside it (rank 0, N = 1 only for the oracle)
+    fma_peak = pk.tkhp_fma_peak(local_rank, precision, args.peak_seconds) if rank == 0 else None
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        rows = 8192 if n > 20000 else n
+        r = oracle_sample(sys_, rows)
+        cpu = {"value": r["pair_interactions"] / r["seconds"], "unit": UNIT, "cores": r["cores"],
+               "kind": "oracle", "seconds": r["seconds"],
+               "sample": f"oracle perm_field + one tmatvec on {r['rows']} seeded random rows of {WORKLOADS[args.config]}"}
+    P.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+    if roofline is not None and fma_peak:
+        roofline["peak_measured_fma_chain"] = fma_peak
+        roofline["frac_of_measured_fma"] = achieved / fma_peak
+        roofline["executed_frac_of_measured_fma"] = executed / fma_peak
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32 pair math, f64 accumulation" if args.precision == "mixed" else "f64",
+        "data": "synthetic",
+        "config": {"workload": WORKLOADS[args.config], "n_atoms": n, "box": sys_.box,
+                   "cutoff": sys_.cutoff, "skin": sys_.skin, "ewald_beta": sys_.ewald_beta,
+                   "tol": args.tol, "precision": args.precision,
+                   "list_mode": "cluster" if mode_in_use == pk.TKHP_LIST_CLUSTER else "tiles",
+                   "parallelism": "replicas x%d" % world, "l2": "flushed between timed steps (256 MiB fill)"},
+        "n_pair_within_cutoff": n_pair, "pcg_iterations": statistics.mean(iters),
+        "pair_interactions_per_step": pairs_per_step, "energy_kcal_mol": energy, "final_rms": rms,
+        "phase_ms": phase_ms,
+        "wall_ms_per_step_incl_flush": 1e3 * wall_s / args.steps,
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+        "gpu_launches": prof_tot["launches"], "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world == 1 and args.gpus > 1 and args.impl == "ours":
+        # plain `python bench.py --gpus N`: re-launch under torchrun, one rank per GPU
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", "29531", str(Path(__file__).resolve())] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -177,6 +177,20 @@ int tkhp_polarize_host(tkhp_ctx *ctx, const double *h_pos, const double *h_polar
 int tkhp_last_timings(tkhp_ctx *ctx, double ms[5]);
 
 /*
+ * Launch accounting and live kernel timing for benchmarks.
+ * tkhp_profile_reset zeroes the launch counter; with enable_kernel_events != 0 every later
+ * T.mu / field PAIR kernel launch (at most 64 of each until the next reset) is bracketed by
+ * its own CUDA event pair on the launching stream.  tkhp_profile_read synchronises those
+ * events and returns: kernels launched by this context since the reset (every __global__
+ * launch of libtkhp; memsets and copies are not kernels), the number of recorded T.mu pair
+ * kernel launches and their summed duration in ms, the same for the field pair kernel.
+ * Any output pointer may be NULL.
+ */
+int tkhp_profile_reset(tkhp_ctx *ctx, int32_t enable_kernel_events);
+int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmatvec_kernels,
+                      double *tmatvec_kernel_ms, int32_t *n_field_kernels, double *field_kernel_ms);
+
+/*
  * Register-resident FMA microbenchmark used as the measured ALU roofline denominator
  * (SURVEY 8(d) "Peaks"): runs dependent-chain FMAs with 8 accumulators per thread on every
  * SM for about `seconds`, returns sustained TFLOP/s (2 flops per FMA).

@@ -15,7 +15,7 @@ from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_LIST_TILES, TKHP_LIST_CLUSTER,
                       tkhp_nblist_build, tkhp_nblist_view, tkhp_nblist_stats,
                       tkhp_perm_field, tkhp_tmatvec, tkhp_polar_solve,
                       tkhp_polar_energy, tkhp_polarize_host, tkhp_last_timings,
-                      tkhp_fma_peak, EXPORTED_SYMBOLS)
+                      tkhp_fma_peak, tkhp_profile_reset, tkhp_profile_read, EXPORTED_SYMBOLS)
 
 __all__ = [
     "TKHP_FP64", "TKHP_MIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TkhpError",
@@ -23,5 +23,5 @@ __all__ = [
     "tkhp_destroy", "tkhp_last_error", "tkhp_nblist_build", "tkhp_nblist_view",
     "tkhp_nblist_stats", "tkhp_perm_field", "tkhp_tmatvec", "tkhp_polar_solve",
     "tkhp_polar_energy", "tkhp_polarize_host", "tkhp_last_timings", "tkhp_fma_peak",
-    "EXPORTED_SYMBOLS",
+    "tkhp_profile_reset", "tkhp_profile_read", "EXPORTED_SYMBOLS",
 ]

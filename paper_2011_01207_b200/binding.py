@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "tkhp_workspace_bytes", "tkhp_create", "tkhp_destroy", "tkhp_last_error",
     "tkhp_nblist_build", "tkhp_nblist_view", "tkhp_nblist_stats", "tkhp_perm_field",
     "tkhp_tmatvec", "tkhp_polar_solve", "tkhp_polar_energy", "tkhp_polarize_host",
-    "tkhp_last_timings", "tkhp_fma_peak",
+    "tkhp_last_timings", "tkhp_fma_peak", "tkhp_profile_reset", "tkhp_profile_read",
 ]
 
 
@@ -74,6 +74,9 @@ def lib() -> ctypes.CDLL:
                                          vp, vp, vp, POINTER(c_int32), POINTER(c_double), vp]
         L.tkhp_last_timings.argtypes = [c_void_p, POINTER(c_double)]
         L.tkhp_fma_peak.argtypes = [c_int32, c_int32, c_double, POINTER(c_double)]
+        L.tkhp_profile_reset.argtypes = [c_void_p, c_int32]
+        L.tkhp_profile_read.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int32),
+                                        POINTER(c_double), POINTER(c_int32), POINTER(c_double)]
         for name in EXPORTED_SYMBOLS:
             if name != "tkhp_last_error":
                 getattr(L, name).restype = ctypes.c_int
@@ -199,6 +202,19 @@ def tkhp_last_timings(ctx):
     arr = (c_double * 5)()
     _check(lib().tkhp_last_timings(ctx, arr), ctx)
     return dict(zip(("build", "field", "tmatvec", "solve", "energy"), list(arr)))
+
+
+def tkhp_profile_reset(ctx, enable_kernel_events: bool = True):
+    _check(lib().tkhp_profile_reset(ctx, 1 if enable_kernel_events else 0), ctx)
+
+
+def tkhp_profile_read(ctx):
+    """-> dict(launches, n_tmatvec, tmatvec_ms, n_field, field_ms)."""
+    nl, nt, nf = c_int64(0), c_int32(0), c_int32(0)
+    tt, tf = c_double(0.0), c_double(0.0)
+    _check(lib().tkhp_profile_read(ctx, byref(nl), byref(nt), byref(tt), byref(nf), byref(tf)), ctx)
+    return dict(launches=nl.value, n_tmatvec=nt.value, tmatvec_ms=tt.value, n_field=nf.value,
+                field_ms=tf.value)
 
 
 def tkhp_fma_peak(device: int, precision: int, seconds: float = 2.0) -> float:

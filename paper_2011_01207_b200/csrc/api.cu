@@ -197,6 +197,8 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
         return TKHP_ECUDA;
     }
     for (int i = 0; i < 10; ++i) cudaEventCreate(&c->ev[i]);
+    for (int w = 0; w < 2; ++w)
+        for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventCreate(&c->prof_ev[w][i]);
     for (int i = 0; i < 5; ++i) c->last_ms[i] = -1.0;
     c->built = false;
     c->header_valid = false;
@@ -212,6 +214,8 @@ int tkhp_destroy(tkhp_ctx *ctx) {
     cudaSetDevice(c->p.device);
     cudaDeviceSynchronize();
     for (int i = 0; i < 10; ++i) cudaEventDestroy(c->ev[i]);
+    for (int w = 0; w < 2; ++w)
+        for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventDestroy(c->prof_ev[w][i]);
     cudaFreeHost(c->h_scalars);
     cudaFreeHost(c->h_state);
     delete c;
@@ -364,6 +368,39 @@ int tkhp_polarize_host(tkhp_ctx *ctx, const double *h_pos, const double *h_polar
     TKHP_CUDA(c, cudaMemcpyAsync(h_energy, c->h_energy, 8, cudaMemcpyDeviceToHost, s));
     TKHP_CUDA(c, cudaStreamSynchronize(s));
     return rc_solve;
+}
+
+int tkhp_profile_reset(tkhp_ctx *ctx, int32_t enable_kernel_events) {
+    if (!ctx) return TKHP_EINVAL;
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    c->n_launches = 0;
+    c->prof = enable_kernel_events != 0;
+    c->prof_n[0] = c->prof_n[1] = 0;
+    return TKHP_OK;
+}
+
+int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmatvec_kernels,
+                      double *tmatvec_kernel_ms, int32_t *n_field_kernels, double *field_kernel_ms) {
+    if (!ctx) return TKHP_EINVAL;
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (n_kernel_launches) *n_kernel_launches = c->n_launches;
+    double tot[2] = {0.0, 0.0};
+    for (int w = 0; w < 2; ++w) {
+        for (int i = 0; i < c->prof_n[w]; ++i) {
+            float t = 0.f;
+            if (cudaEventSynchronize(c->prof_ev[w][2 * i + 1]) != cudaSuccess ||
+                cudaEventElapsedTime(&t, c->prof_ev[w][2 * i], c->prof_ev[w][2 * i + 1]) != cudaSuccess) {
+                cudaGetLastError();
+                return set_err(c, TKHP_ECUDA, "profile events not complete%s");
+            }
+            tot[w] += t;
+        }
+    }
+    if (n_tmatvec_kernels) *n_tmatvec_kernels = c->prof_n[0];
+    if (tmatvec_kernel_ms) *tmatvec_kernel_ms = tot[0];
+    if (n_field_kernels) *n_field_kernels = c->prof_n[1];
+    if (field_kernel_ms) *field_kernel_ms = tot[1];
+    return TKHP_OK;
 }
 
 int tkhp_last_timings(tkhp_ctx *ctx, double ms[5]) {

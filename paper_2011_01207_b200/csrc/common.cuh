@@ -107,7 +107,13 @@ struct Ctx {
 
     cudaEvent_t ev[10];
     double last_ms[5];
+    // launch accounting / live kernel timing (tkhp_profile_*)
+    long long n_launches;               // kernels launched since the last reset
+    bool prof;                          // record an event pair around every T.mu / field pair kernel
+    int prof_n[2];                      // [0] T.mu launches, [1] field launches recorded
+    cudaEvent_t prof_ev[2][2 * 64];
 };
+constexpr int PROF_MAX = 64;
 
 // Bump allocator over the caller's workspace; with base == nullptr it only measures.
 struct Carver {

@@ -97,7 +97,8 @@ __global__ void k_scan_apply(const uint32_t *__restrict__ in, uint32_t n,
 }
 
 // out[i] = sum_{k<i} in[k], i = 0..n-1 (so pass n = bins + 1 to get the grand total at out[bins]).
-static void exclusive_scan(const uint32_t *in, uint32_t *out, uint32_t n, uint32_t *tmp, cudaStream_t s) {
+static void exclusive_scan(Ctx *c, const uint32_t *in, uint32_t *out, uint32_t n, uint32_t *tmp, cudaStream_t s) {
+    c->n_launches += 3;
     uint32_t nb = (n + SCAN_TILE - 1) / SCAN_TILE;
     k_scan_reduce<<<nb, SCAN_THREADS, 0, s>>>(in, n, tmp);
     k_scan_sums<<<1, SCAN_THREADS, 0, s>>>(tmp, nb);
@@ -281,9 +282,10 @@ __global__ void k_fill_i32(int32_t *p, int n, int32_t v) {
 }
 
 // sort indices 0..n-1 by (key, index); start[0..n_bins] = bin offsets (kept for the groups)
-static void counting_sort(const uint32_t *key, int n, uint32_t n_bins, uint32_t *count, uint32_t *start,
+static void counting_sort(Ctx *c, const uint32_t *key, int n, uint32_t n_bins, uint32_t *count, uint32_t *start,
                           uint32_t *scan_tmp, int32_t *tmp_idx, int32_t *out_idx, cudaStream_t s) {
-    exclusive_scan(count, start, n_bins + 1, scan_tmp, s);
+    exclusive_scan(c, count, start, n_bins + 1, scan_tmp, s);
+    c->n_launches += 2;
     int nb = div_up(n, 256);
     k_bin_scatter<<<nb, 256, 0, s>>>(key, n, start, count, tmp_idx);
     k_bin_rank<<<nb, 256, 0, s>>>(key, n, start, tmp_idx, out_idx);
@@ -488,23 +490,25 @@ int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32
     if (p.box > 0.0) {
         const int b = c->grid_bits_host;
         k_state_init<<<1, 1, 0, s>>>(c->st, b, (double)(1 << b) / p.box);
+        c->n_launches += 1;
     } else {
         k_state_init<<<1, 1, 0, s>>>(c->st, 1, 1.0);
         k_extent<<<nb256, 256, 0, s>>>(d_pos, n, c->st);
         int b_max = 0;
         while ((1 << (3 * (b_max + 1))) <= c->n_cells_alloc) ++b_max;
         k_grid_from_extent<<<1, 1, 0, s>>>(c->st, b_max);
+        c->n_launches += 3;
     }
     TKHP_CUDA(c, cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * ((size_t)c->n_cells_alloc + 1), s));
     k_cell_keys<<<nb256, 256, 0, s>>>(d_pos, d_alpha, d_group, n, p.box, c->st, c->key, c->cell_count);
-    counting_sort(c->key, n, (uint32_t)c->n_cells_alloc, c->cell_count, c->cell_start, c->scan_tmp,
+    counting_sort(c, c->key, n, (uint32_t)c->n_cells_alloc, c->cell_count, c->cell_start, c->scan_tmp,
                   c->tmp_idx, c->perm, s);
-    if (c->n_pad > n) k_fill_i32<<<1, 32, 0, s>>>(c->perm + n, c->n_pad - n, -1);
+    if (c->n_pad > n) { k_fill_i32<<<1, 32, 0, s>>>(c->perm + n, c->n_pad - n, -1); c->n_launches += 1; }
 
     // polarization groups: members sorted by (group, index)
     TKHP_CUDA(c, cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * ((size_t)n + 1), s));
     k_group_keys<<<nb256, 256, 0, s>>>(d_group, n, c->key, c->cell_count);
-    counting_sort(c->key, n, (uint32_t)n, c->cell_count, c->grp_start, c->scan_tmp, c->tmp_idx,
+    counting_sort(c, c->key, n, (uint32_t)n, c->cell_count, c->grp_start, c->scan_tmp, c->tmp_idx,
                   c->grp_members, s);
 
     // gather + boxes
@@ -525,11 +529,12 @@ int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32
         c->bcentre, c->bhalf, c->scentre, c->shalf, c->n_blocks, c->n_super, p.box, reach2, reach2_super,
         c->row_count, c->row_start, c->pairs, c->cap_tiles, c->st);
     TKHP_CUDA(c, cudaMemsetAsync(c->row_count + c->n_blocks, 0, sizeof(uint32_t), s));
-    exclusive_scan(c->row_count, c->row_start, (uint32_t)c->n_blocks + 1, c->scan_tmp, s);
+    exclusive_scan(c, c->row_count, c->row_start, (uint32_t)c->n_blocks + 1, c->scan_tmp, s);
     k_pair_search<true><<<grid_rows, warps_per_cta * 32, 0, s>>>(
         c->bcentre, c->bhalf, c->scentre, c->shalf, c->n_blocks, c->n_super, p.box, reach2, reach2_super,
         c->row_count, c->row_start, c->pairs, c->cap_tiles, c->st);
     k_list_finish<<<1, 1, 0, s>>>(c->st, c->row_start, c->n_blocks, c->cap_tiles, p.box, p.cutoff);
+    c->n_launches += 7;   // cell keys, group keys, gather, super boxes, 2 x pair search, finish
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }

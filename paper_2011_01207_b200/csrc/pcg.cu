@@ -289,13 +289,30 @@ static inline int vec_grid(const Ctx *c) {
     return g < MAX_PARTIALS ? g : MAX_PARTIALS;
 }
 
+// live kernel timing: one event pair around the pair kernel alone (not the memset)
+static inline bool prof_begin(Ctx *c, int which, cudaStream_t s) {
+    if (!c->prof || c->prof_n[which] >= PROF_MAX) return false;
+    cudaEventRecord(c->prof_ev[which][2 * c->prof_n[which]], s);
+    return true;
+}
+static inline void prof_end(Ctx *c, int which, cudaStream_t s) {
+    cudaEventRecord(c->prof_ev[which][2 * c->prof_n[which] + 1], s);
+    c->prof_n[which]++;
+}
+
 int run_tmatvec(Ctx *c, cudaStream_t s) {
     TKHP_CUDA(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 3 * (size_t)c->n_pad, s));
-    return c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_tmatvec(c, s) : tiles_tmatvec(c, s);
+    const bool rec = prof_begin(c, 0, s);
+    int rc = c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_tmatvec(c, s) : tiles_tmatvec(c, s);
+    if (rec) prof_end(c, 0, s);
+    return rc;
 }
 int run_field(Ctx *c, cudaStream_t s) {
     TKHP_CUDA(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 3 * (size_t)c->n_pad, s));
-    return c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_field(c, s) : tiles_field(c, s);
+    const bool rec = prof_begin(c, 1, s);
+    int rc = c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_field(c, s) : tiles_field(c, s);
+    if (rec) prof_end(c, 1, s);
+    return rc;
 }
 
 int do_perm_field(Ctx *c, const double *d_q, const double *d_dip, const double *d_quad, double *d_field,
@@ -305,6 +322,7 @@ int do_perm_field(Ctx *c, const double *d_q, const double *d_dip, const double *
         k_pack_multipoles<float4><<<g, VEC_THREADS, 0, s>>>(d_q, d_dip, d_quad, c->group_o, c->perm, c->n_pad, c->mp32);
     else
         k_pack_multipoles<double4><<<g, VEC_THREADS, 0, s>>>(d_q, d_dip, d_quad, c->group_o, c->perm, c->n_pad, c->mp64);
+    c->n_launches += 2;   // pack, finish
     int rc = run_field(c, s);
     if (rc) return rc;
     k_field_finish<<<g, VEC_THREADS, 0, s>>>(c->acc, c->perm, c->n_pad, c->pos_o, c->group_o, c->grp_start,
@@ -320,6 +338,7 @@ int do_tmatvec(Ctx *c, const double *d_mu, double *d_out, cudaStream_t s) {
         k_pack_mu_user<float4><<<g, VEC_THREADS, 0, s>>>(d_mu, c->perm, c->n_pad, c->mu32);
     else
         k_pack_mu_user<double4><<<g, VEC_THREADS, 0, s>>>(d_mu, c->perm, c->n_pad, c->mu64);
+    c->n_launches += 2;   // pack, finish
     int rc = run_tmatvec(c, s);
     if (rc) return rc;
     k_tmatvec_finish<<<g, VEC_THREADS, 0, s>>>(c->acc, c->perm, c->n_pad, d_mu, self_coeff(c->p), d_out);
@@ -355,6 +374,7 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
     else
         k_pcg_residual0<double4><<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vE, c->vmu, c->alpha_s, c->inv_alpha_s, self, n_pad, c->vr, c->vp, c->mu64, part_rz[0]);
     k_publish_rr<<<1, VEC_THREADS, 0, s>>>(part_rz[0], gv, c->st);
+    c->n_launches += 3;   // init, residual0, publish
     double rr;
     if ((rc = read_rr(c, s, &rr))) return rc;
     double rms = sqrt(rr / c->n);
@@ -368,12 +388,14 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
             k_pcg_direction<float4><<<gv, VEC_THREADS, 0, s>>>(part_rz[cur], part_rz[nxt], gv, c->vr, c->alpha_s, n_pad, c->vp, c->mu32, c->st);
         else
             k_pcg_direction<double4><<<gv, VEC_THREADS, 0, s>>>(part_rz[cur], part_rz[nxt], gv, c->vr, c->alpha_s, n_pad, c->vp, c->mu64, c->st);
+        c->n_launches += 3;   // q, update, direction
         ++it;
         if ((rc = read_rr(c, s, &rr))) return rc;
         rms = sqrt(rr / c->n);
         if (!(rms == rms)) break;   // NaN: give up
     }
     k_unsort3<<<g1, VEC_THREADS, 0, s>>>(c->vmu, c->perm, n_pad, d_mu);
+    c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
     TKHP_CUDA(c, cudaStreamSynchronize(s));
     if (h_iters) *h_iters = it;
@@ -389,6 +411,7 @@ int do_polar_energy(Ctx *c, const double *d_mu, const double *d_field, double *d
     double *part = c->partials + 6 * MAX_PARTIALS;
     k_energy_partials<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, part);
     k_energy_final<<<1, VEC_THREADS, 0, s>>>(part, g, d_energy);
+    c->n_launches += 2;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }

@@ -229,6 +229,7 @@ int tiles_tmatvec(Ctx *c, cudaStream_t s) {
         TKHP_LAUNCH_TILES(k_tiles_tmu, float, c->xyzw32, c->mu32);
     else
         TKHP_LAUNCH_TILES(k_tiles_tmu, double, c->xyzw64, c->mu64);
+    c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }
@@ -240,6 +241,7 @@ int tiles_field(Ctx *c, cudaStream_t s) {
         TKHP_LAUNCH_TILES(k_tiles_field, float, c->xyzw32, c->mp32);
     else
         TKHP_LAUNCH_TILES(k_tiles_field, double, c->xyzw64, c->mp64);
+    c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }
