@@ -136,6 +136,7 @@ int ensure_header(Ctx *c, cudaStream_t s) {
         TKHP_CUDA(c, cudaStreamSynchronize(s));
         c->header_valid = true;
         c->n_tiles_host = c->h_state->n_tiles;
+        c->list_mode_in_use = (c->p.list_mode == TKHP_LIST_CLUSTER && !c->h_state->cluster_bad) ? TKHP_LIST_CLUSTER : TKHP_LIST_TILES;
     }
     const DeviceState &h = *c->h_state;
     if (h.err_nonfinite) return set_err(c, TKHP_ENONFINITE, "non-finite position passed to tkhp_nblist_build%s");

@@ -35,7 +35,8 @@ struct DeviceState {
     // geometry
     unsigned long long max_half_bits;   // max block half-extent over all axes (bits of a double >= 0)
     int per_pair_image;                 // 1: box too small for one image shift per tile
-    int cluster_ok;                     // 1: CLUSTER lists valid for this geometry
+    int cluster_bad;                    // 1: CLUSTER lists unusable (box too small / capacity): TILES are used
+    int max_stage;                      // largest staged-atom count of any group (CLUSTER mode)
     // list sizes
     long long n_tiles;                  // block pairs kept
     long long n_diag_tiles;

@@ -301,7 +301,9 @@ static inline void prof_end(Ctx *c, int which, cudaStream_t s) {
 }
 
 int run_tmatvec(Ctx *c, cudaStream_t s) {
-    TKHP_CUDA(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 3 * (size_t)c->n_pad, s));
+    // the tile kernel accumulates with atomics into zeroed accumulators; the cluster kernel stores
+    if (c->list_mode_in_use != TKHP_LIST_CLUSTER)
+        TKHP_CUDA(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 3 * (size_t)c->n_pad, s));
     const bool rec = prof_begin(c, 0, s);
     int rc = c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_tmatvec(c, s) : tiles_tmatvec(c, s);
     if (rec) prof_end(c, 0, s);

@@ -39,6 +39,8 @@ SYSTEMS = {
     "n65_periodic": lambda: tiny_cluster(65, 4, box=14.0, spread=14.0, cutoff=5.0, skin=1.0, ewald_beta=0.6),
     "n200_periodic_noewald": lambda: tiny_cluster(200, 5, box=20.0, spread=20.0, cutoff=6.0, skin=1.0),
     "water_1536_solutes": lambda: water_box(512, 24.85, 77, solute_frac=0.15),
+    # large enough for the CLUSTER lists (box/2 > cutoff + group extent), small enough for Cholesky
+    "water_6000": lambda: water_box(2000, 39.2, 78, solute_frac=0.1),
 }
 
 
@@ -80,29 +82,52 @@ def test_nblist_is_deterministic_and_rebuildable():
 
 
 # ------------------------------------------------------------------ T.mu and field
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
 @pytest.mark.parametrize("precision", ["fp64", "mixed"])
-def test_tmatvec_matches_oracle(system, precision):
+def test_tmatvec_matches_oracle(system, precision, list_mode):
     s = system
     rng = np.random.default_rng(42)
     mu = rng.standard_normal((s.n_atoms, 3)) * 0.1
     want = oracle.tmatvec(s, mu)
-    P = _polarizer(s, precision)
+    P = _polarizer(s, precision, list_mode)
     got = P.tmatvec(mu).cpu().numpy()
     assert _rel_l2(got, want) <= TOL_VEC[precision]
     P.close()
 
 
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
 @pytest.mark.parametrize("precision", ["fp64", "mixed"])
-def test_perm_field_matches_oracle(system, precision):
+def test_perm_field_matches_oracle(system, precision, list_mode):
     s = system
     want = oracle.perm_field(s)
-    P = _polarizer(s, precision)
+    P = _polarizer(s, precision, list_mode)
     got = P.perm_field(s.charge, s.dipole, s.quad).cpu().numpy()
     if np.linalg.norm(want) < 1e-12:      # isolated masked molecule: field is zero up to rounding
         assert np.abs(got).max() < 1e-12
     else:
         assert _rel_l2(got, want) <= TOL_VEC[precision]
     P.close()
+
+
+def test_cluster_mode_is_used_and_deterministic():
+    """CLUSTER lists are active on a big enough box, fall back to TILES on a small one, and the
+    cluster kernel (no atomics) returns bit-identical results run to run."""
+    pk = _pk()
+    s = SYSTEMS["water_6000"]()
+    P = _polarizer(s, "mixed", "cluster")
+    n_pair, n_slots, mode = P.nblist_stats()
+    assert mode == pk.TKHP_LIST_CLUSTER and n_pair == oracle.count_pairs(s)
+    assert 2 * n_pair <= n_slots <= 8 * n_pair          # ordered useful slots <= executed slots
+    rng = np.random.default_rng(3)
+    mu = rng.standard_normal((s.n_atoms, 3))
+    a = P.tmatvec(mu).cpu().numpy()
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    b = P.tmatvec(mu).cpu().numpy()
+    assert np.array_equal(a, b)
+    P.close()
+    small = _polarizer(make_config(0), "mixed", "cluster")
+    assert small.nblist_stats()[2] == pk.TKHP_LIST_TILES
+    small.close()
 
 
 def test_tmatvec_symmetry_on_gpu():
@@ -119,16 +144,17 @@ def test_tmatvec_symmetry_on_gpu():
 
 
 # ------------------------------------------------------------------ solve and energy
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
 @pytest.mark.parametrize("precision", ["fp64", "mixed"])
-@pytest.mark.parametrize("name", ["cfg0", "n65_periodic", "water_1536_solutes"])
-def test_solve_and_energy_match_oracle(name, precision):
+@pytest.mark.parametrize("name", ["cfg0", "n65_periodic", "water_1536_solutes", "water_6000"])
+def test_solve_and_energy_match_oracle(name, precision, list_mode):
     """Q11: both sides converge tighter than the parity bar so that truncation error does not
     mask arithmetic error (oracle: dense Cholesky; GPU: 1e-12 FP64 / 1e-8 MIXED)."""
     s = SYSTEMS[name]()
     E = oracle.perm_field(s)
     mu_ref = oracle.dense_solve(s, E)
     e_ref = oracle.polar_energy(mu_ref, E)
-    P = _polarizer(s, precision)
+    P = _polarizer(s, precision, list_mode)
     Eg = P.perm_field(s.charge, s.dipole, s.quad)
     tol = 1e-12 if precision == "fp64" else 1e-8
     mu, it, rms = P.polar_solve(Eg, tol=tol, max_iter=100)
