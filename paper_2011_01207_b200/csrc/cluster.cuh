@@ -1,0 +1,116 @@
+// cluster.cuh / cluster_build.cu / cluster_pairs.cu -- CLUSTER list mode: filtered cluster->atom lists with the neighbourhood of a
+// group of blocks staged in shared memory.
+//
+// Paper, "List filtering": "By filtering every neighboring group, we can get a list
+// of atoms which really belong to a group's neighborhood ... alpha in B_I if there is alpha_i in
+// beta_I such that dist(alpha_i, alpha) <= d_cut + d_buff ... phantom atoms to complete the actual
+// neighbor lists ... a loss of coalesced memory access pattern ... compensated by an increase of
+// B_comp", +75% on their vdW kernel, then applied to "electrostatics and polarization".
+//
+// B200 redesign:
+//  * the filter granularity is an 8-atom CLUSTER (a quarter warp), not the 32-atom block: with
+//    r_c = 7 A a 32-atom block is as wide as the cutoff and only ~26% of (block atom, list atom)
+//    slots are inside r_c; for 8-atom clusters it is ~49% (measured, DESIGN.md table 5.1);
+//  * the filter radius is r_c (+0.01 A guard), not r_c + skin: the list is used for the positions
+//    it was built from (one solve), the skin only enters the prescribed block-pair list;
+//  * a CTA owns a GROUP of up to 8 consecutive blocks; every list atom of the group's clusters is
+//    staged ONCE in shared memory (position already shifted into the group's frame, so no image
+//    arithmetic in the pair loop), and list entries are 16-bit indices into that staging area:
+//    the "loss of coalesced access" the paper notes becomes conflict-free LDS.128 (each quarter
+//    warp reads one 16-byte record, broadcast to its 8 lanes);
+//  * every lane owns one atom i and only ever updates atom i: no atomics, no j-side accumulator,
+//    bit-reproducible results; FP32 partials are flushed into FP64 registers every 32 entries
+//    (64-bit containers for accumulation);
+//  * the number of groups is a whole multiple of (SM count x resident CTAs) whenever the system
+//    is smaller than a few waves, so every SM gets the same number of blocks.
+#pragma once
+#include "common.cuh"
+#include "pair_math.cuh"
+
+namespace tkhp {
+
+constexpr int GB = 8;                 // max blocks per group (= warps per CTA)
+constexpr int GT = GB * 32;           // threads per CTA
+constexpr int OCT = GB * 4;           // clusters per group
+constexpr int CB_CAP = 1024;          // candidate blocks per group
+constexpr int RESIDENT = 3;           // CTAs per SM the group count is rounded to
+constexpr int B200_SMS = 148;
+constexpr float GUARD = 0.01f;        // list radius = r_c + GUARD (FP32 build arithmetic is safe)
+
+struct ClusterWs {
+    int n_groups, s_cap, l_cap;
+    int32_t *group_first;             // n_groups + 1
+    float4 *gpos32;                   // n_pad: atom in its group's frame (x,y,z,w)
+    double4 *gpos64;
+    int32_t *stage_count;             // n_groups
+    int32_t *stage_atom;              // n_groups * s_cap: sorted slot of each staged atom
+    float4 *stage_pos32;              // n_groups * s_cap: position in the group's frame (+w)
+    double4 *stage_pos64;
+    uint32_t *stage_mask;             // n_groups * s_cap: which clusters of the group list the atom
+    uint16_t *entries;                // (n_pad/8) * l_cap
+    int32_t *oct_len;                 // n_pad/8: padded list length (equal within a warp)
+};
+
+inline int choose_groups(int n_blocks) {
+    const int base = (n_blocks + GB - 1) / GB;
+    const int wave = B200_SMS * RESIDENT;
+    if (base >= 4 * wave) return base;
+    int g = ((base + wave - 1) / wave) * wave;
+    if (g > n_blocks) g = n_blocks;
+    return g;
+}
+
+inline void size_caps(const tkhp_params *p, int n_blocks, int *s_cap, int *l_cap) {
+    const long long n_pad = (long long)n_blocks * BLOCK;
+    long long s, l;
+    if (p->box > 0.0) {
+        const double rho = p->n_atoms / (p->box * p->box * p->box);
+        const double e = 1.3 * cbrt(GT / rho);
+        double edge = e + 2.0 * (p->cutoff + 1.0);
+        if (edge > p->box) edge = p->box;
+        s = (long long)(1.25 * edge * edge * edge * rho) + 64;
+        const double r = p->cutoff + 3.0;
+        l = (long long)(1.5 * 4.18879 * r * r * r * rho) + 64;
+    } else {
+        s = 8192;
+        l = 2048;
+    }
+    if (p->max_nbrs_per_cluster > 0) l = p->max_nbrs_per_cluster;
+    if (s > n_pad + 1) s = n_pad + 1;
+    if (l > n_pad + 8) l = n_pad + 8;
+    if (s > 65535) s = 65535;          // 16-bit entries
+    *s_cap = (int)((s + 63) & ~63LL);
+    *l_cap = (int)((l + 7) & ~7LL);
+}
+
+inline size_t carve_cluster(const tkhp_params *p, int n_blocks, void *base, ClusterWs *out) {
+    Carver w(base);
+    ClusterWs ws;
+    const size_t n_pad = (size_t)n_blocks * BLOCK;
+    ws.n_groups = choose_groups(n_blocks);
+    size_caps(p, n_blocks, &ws.s_cap, &ws.l_cap);
+    const bool f64 = p->precision == TKHP_FP64;
+    const size_t gs = (size_t)ws.n_groups * ws.s_cap;
+    ws.group_first = w.take<int32_t>(ws.n_groups + 1);
+    ws.gpos32 = w.take<float4>(n_pad);
+    ws.gpos64 = f64 ? w.take<double4>(n_pad) : nullptr;
+    ws.stage_count = w.take<int32_t>(ws.n_groups);
+    ws.stage_atom = w.take<int32_t>(gs);
+    ws.stage_pos32 = w.take<float4>(gs);
+    ws.stage_pos64 = f64 ? w.take<double4>(gs) : nullptr;
+    ws.stage_mask = w.take<uint32_t>(gs);
+    ws.entries = w.take<uint16_t>((n_pad / CLUSTER) * ws.l_cap);
+    ws.oct_len = w.take<int32_t>(n_pad / CLUSTER);
+    w.take<char>(256);
+    if (out) *out = ws;
+    return w.off;
+}
+
+
+inline ClusterWs get_ws(Ctx *c) {
+    ClusterWs ws;
+    carve_cluster(&c->p, c->n_blocks, c->cl_ws, &ws);
+    return ws;
+}
+
+}  // namespace tkhp

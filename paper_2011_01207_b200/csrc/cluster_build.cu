@@ -1,120 +1,7 @@
-// cluster.cu -- CLUSTER list mode: filtered cluster->atom lists with the neighbourhood of a
-// group of blocks staged in shared memory.
-//
-// Paper, "List filtering": "By filtering every neighboring group, we can get a list
-// of atoms which really belong to a group's neighborhood ... alpha in B_I if there is alpha_i in
-// beta_I such that dist(alpha_i, alpha) <= d_cut + d_buff ... phantom atoms to complete the actual
-// neighbor lists ... a loss of coalesced memory access pattern ... compensated by an increase of
-// B_comp", +75% on their vdW kernel, then applied to "electrostatics and polarization".
-//
-// B200 redesign:
-//  * the filter granularity is an 8-atom CLUSTER (a quarter warp), not the 32-atom block: with
-//    r_c = 7 A a 32-atom block is as wide as the cutoff and only ~26% of (block atom, list atom)
-//    slots are inside r_c; for 8-atom clusters it is ~49% (measured, DESIGN.md table 5.1);
-//  * the filter radius is r_c (+0.01 A guard), not r_c + skin: the list is used for the positions
-//    it was built from (one solve), the skin only enters the prescribed block-pair list;
-//  * a CTA owns a GROUP of up to 8 consecutive blocks; every list atom of the group's clusters is
-//    staged ONCE in shared memory (position already shifted into the group's frame, so no image
-//    arithmetic in the pair loop), and list entries are 16-bit indices into that staging area:
-//    the "loss of coalesced access" the paper notes becomes conflict-free LDS.128 (each quarter
-//    warp reads one 16-byte record, broadcast to its 8 lanes);
-//  * every lane owns one atom i and only ever updates atom i: no atomics, no j-side accumulator,
-//    bit-reproducible results; FP32 partials are flushed into FP64 registers every 32 entries
-//    (64-bit containers for accumulation);
-//  * the number of groups is a whole multiple of (SM count x resident CTAs) whenever the system
-//    is smaller than a few waves, so every SM gets the same number of blocks.
-#include "common.cuh"
-#include "pair_math.cuh"
+// cluster_build.cu -- construction of the CLUSTER lists (see cluster.cuh for the design).
+#include "cluster.cuh"
 
 namespace tkhp {
-
-constexpr int GB = 8;                 // max blocks per group (= warps per CTA)
-constexpr int GT = GB * 32;           // threads per CTA
-constexpr int OCT = GB * 4;           // clusters per group
-constexpr int CB_CAP = 1024;          // candidate blocks per group
-constexpr int RESIDENT = 3;           // CTAs per SM the group count is rounded to
-constexpr int B200_SMS = 148;
-constexpr float GUARD = 0.01f;        // list radius = r_c + GUARD (FP32 build arithmetic is safe)
-
-struct ClusterWs {
-    int n_groups, s_cap, l_cap;
-    int32_t *group_first;             // n_groups + 1
-    float4 *gpos32;                   // n_pad: atom in its group's frame (x,y,z,w)
-    double4 *gpos64;
-    int32_t *stage_count;             // n_groups
-    int32_t *stage_atom;              // n_groups * s_cap: sorted slot of each staged atom
-    float4 *stage_pos32;              // n_groups * s_cap: position in the group's frame (+w)
-    double4 *stage_pos64;
-    uint32_t *stage_mask;             // n_groups * s_cap: which clusters of the group list the atom
-    uint16_t *entries;                // (n_pad/8) * l_cap
-    int32_t *oct_len;                 // n_pad/8: padded list length (equal within a warp)
-};
-
-static int choose_groups(int n_blocks) {
-    const int base = (n_blocks + GB - 1) / GB;
-    const int wave = B200_SMS * RESIDENT;
-    if (base >= 4 * wave) return base;
-    int g = ((base + wave - 1) / wave) * wave;
-    if (g > n_blocks) g = n_blocks;
-    return g;
-}
-
-static void size_caps(const tkhp_params *p, int n_blocks, int *s_cap, int *l_cap) {
-    const long long n_pad = (long long)n_blocks * BLOCK;
-    long long s, l;
-    if (p->box > 0.0) {
-        const double rho = p->n_atoms / (p->box * p->box * p->box);
-        const double e = 1.3 * cbrt(GT / rho);
-        double edge = e + 2.0 * (p->cutoff + 1.0);
-        if (edge > p->box) edge = p->box;
-        s = (long long)(1.25 * edge * edge * edge * rho) + 64;
-        const double r = p->cutoff + 3.0;
-        l = (long long)(1.5 * 4.18879 * r * r * r * rho) + 64;
-    } else {
-        s = 8192;
-        l = 2048;
-    }
-    if (p->max_nbrs_per_cluster > 0) l = p->max_nbrs_per_cluster;
-    if (s > n_pad + 1) s = n_pad + 1;
-    if (l > n_pad + 8) l = n_pad + 8;
-    if (s > 65535) s = 65535;          // 16-bit entries
-    *s_cap = (int)((s + 63) & ~63LL);
-    *l_cap = (int)((l + 7) & ~7LL);
-}
-
-static size_t carve_cluster(const tkhp_params *p, int n_blocks, void *base, ClusterWs *out) {
-    Carver w(base);
-    ClusterWs ws;
-    const size_t n_pad = (size_t)n_blocks * BLOCK;
-    ws.n_groups = choose_groups(n_blocks);
-    size_caps(p, n_blocks, &ws.s_cap, &ws.l_cap);
-    const bool f64 = p->precision == TKHP_FP64;
-    const size_t gs = (size_t)ws.n_groups * ws.s_cap;
-    ws.group_first = w.take<int32_t>(ws.n_groups + 1);
-    ws.gpos32 = w.take<float4>(n_pad);
-    ws.gpos64 = f64 ? w.take<double4>(n_pad) : nullptr;
-    ws.stage_count = w.take<int32_t>(ws.n_groups);
-    ws.stage_atom = w.take<int32_t>(gs);
-    ws.stage_pos32 = w.take<float4>(gs);
-    ws.stage_pos64 = f64 ? w.take<double4>(gs) : nullptr;
-    ws.stage_mask = w.take<uint32_t>(gs);
-    ws.entries = w.take<uint16_t>((n_pad / CLUSTER) * ws.l_cap);
-    ws.oct_len = w.take<int32_t>(n_pad / CLUSTER);
-    w.take<char>(256);
-    if (out) *out = ws;
-    return w.off;
-}
-
-size_t cluster_workspace_bytes(const tkhp_params *p, int n_blocks) {
-    if (p->list_mode != TKHP_LIST_CLUSTER) return 0;
-    return carve_cluster(p, n_blocks, nullptr, nullptr);
-}
-
-static ClusterWs get_ws(Ctx *c) {
-    ClusterWs ws;
-    carve_cluster(&c->p, c->n_blocks, c->cl_ws, &ws);
-    return ws;
-}
 
 // ----------------------------------------------------------------------------- build
 __global__ void k_group_first(int32_t *group_first, int n_groups, int n_blocks) {
@@ -261,15 +148,17 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
             const float4 p = xyzw32[slot];
             if (p.w > 0.f) {
                 const double4 cj = bcentre[J];
-                double dx = cj.x - gcx, dy = cj.y - gcy, dz = cj.z - gcz;
-                if (box > 0.0) {
-                    dx -= box * rint(dx / box); dy -= box * rint(dy / box); dz -= box * rint(dz / box);
-                }
+                const double dx = cj.x - gcx, dy = cj.y - gcy, dz = cj.z - gcz;
                 if (f64) {
                     const double4 q = xyzw64[slot];
                     px = q.x + dx; py = q.y + dy; pz = q.z + dz; pw = q.w;
                 } else {
                     px = (double)p.x + dx; py = (double)p.y + dy; pz = (double)p.z + dz; pw = p.w;
+                }
+                // the image is chosen per ATOM (unique because r_c + group half extent < box/2);
+                // a per-block shift would be ambiguous when r_c + both extents exceeds box/2
+                if (box > 0.0) {
+                    px -= box * rint(px / box); py -= box * rint(py / box); pz -= box * rint(pz / box);
                 }
                 pj = make_float4((float)px, (float)py, (float)pz, p.w);
                 for (int o = 0; o < OCT; ++o) {
@@ -360,71 +249,11 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
     }
 }
 
-// ----------------------------------------------------------------------------- T.mu
-template <typename real>
-__global__ void __launch_bounds__(GT)
-k_cluster_tmu(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
-              const typename Vec4<real>::type *__restrict__ stage_pos,
-              const typename Vec4<real>::type *__restrict__ mu, PairConsts<real> kc,
-              double *__restrict__ acc, int n_pad, int s_run) {
-    using vec4 = typename Vec4<real>::type;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);
-    vec4 *s_mu = s_pos + s_run;
-
-    const int g = blockIdx.x, t = threadIdx.x, lane = t & 31, w = t >> 5;
-    const int b0 = ws.group_first[g], nb = ws.group_first[g + 1] - b0;
-    const int count = ws.stage_count[g];
-    const size_t gbase = (size_t)g * ws.s_cap;
-    for (int idx = t; idx < count; idx += GT) {
-        s_pos[idx] = stage_pos[gbase + idx];
-        s_mu[idx] = mu[ws.stage_atom[gbase + idx]];
-    }
-    if (t == 0) {
-        vec4 far, zero;
-        far.x = far.y = far.z = (real)(-2.0f * PHANTOM_FAR); far.w = 0;
-        zero.x = zero.y = zero.z = zero.w = 0;
-        s_pos[count] = far;
-        s_mu[count] = zero;
-    }
-    __syncthreads();
-    if (w >= nb) return;
-
-    const int slot = (b0 + w) * BLOCK + lane;
-    const vec4 pi = gpos[slot];
-    const int oct = slot >> 3;
-    const int L = ws.oct_len[oct];
-    const uint16_t *__restrict__ ent = ws.entries + (size_t)oct * ws.l_cap;
-    const int qbase = lane & 24;
-    double dx = 0.0, dy = 0.0, dz = 0.0;
-    real ax = 0, ay = 0, az = 0;
-    for (int k0 = 0; k0 < L; k0 += 8) {
-        const unsigned e = ent[k0 + (lane & 7)];
-#pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-            const unsigned idx = __shfl_sync(0xffffffffu, e, qbase + kk);
-            const vec4 pj = s_pos[idx];
-            const vec4 mj = s_mu[idx];
-            const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
-            const real r2 = Rx * Rx + Ry * Ry + Rz * Rz;
-            const bool in = (r2 <= kc.rc2) && (r2 > (real)1e-10);
-            real G[2];
-            radial<2>(in ? r2 : (real)1, pi.w * pj.w, kc, G);
-            const real m1 = in ? G[0] : (real)0, m2 = in ? G[1] : (real)0;
-            tmu_apply<real>(m1, m2, Rx, Ry, Rz, mj.x, mj.y, mj.z, ax, ay, az);
-        }
-        if ((k0 & 24) == 24) {   // every 32 entries: FP32 partial -> FP64 accumulator
-            dx += (double)ax; dy += (double)ay; dz += (double)az;
-            ax = 0; ay = 0; az = 0;
-        }
-    }
-    dx += (double)ax; dy += (double)ay; dz += (double)az;
-    acc[slot] = dx;
-    acc[n_pad + slot] = dy;
-    acc[2 * (size_t)n_pad + slot] = dz;
+size_t cluster_workspace_bytes(const tkhp_params *p, int n_blocks) {
+    if (p->list_mode != TKHP_LIST_CLUSTER) return 0;
+    return carve_cluster(p, n_blocks, nullptr, nullptr);
 }
 
-// ----------------------------------------------------------------------------- host side
 int cluster_build(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
     k_group_first<<<div_up(ws.n_groups + 1, 256), 256, 0, s>>>(ws.group_first, ws.n_groups, c->n_blocks);
@@ -433,43 +262,6 @@ int cluster_build(Ctx *c, cudaStream_t s) {
     c->n_launches += 2;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
-}
-
-template <typename real>
-static int launch_tmu(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
-    using vec4 = typename Vec4<real>::type;
-    const int s_run = ((c->h_state->max_stage + 1) + 15) & ~15;
-    const size_t smem = 2 * sizeof(vec4) * (size_t)s_run;
-    if (smem > 227 * 1024) return set_err(c, TKHP_ECAPACITY, "cluster staging exceeds shared memory%s");
-    static size_t configured[2] = {0, 0};
-    const int which = sizeof(real) == 8;
-    if (smem > configured[which]) {
-        TKHP_CUDA(c, cudaFuncSetAttribute(k_cluster_tmu<real>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024)));
-        configured[which] = 227 * 1024;
-    }
-    PairConsts<real> k;
-    k.beta = (real)c->p.ewald_beta;
-    k.c1 = (real)(2.0 / SQRT_PI);
-    k.rc2 = (real)(c->p.cutoff * c->p.cutoff);
-    k.box = (real)1; k.inv_box = (real)0;
-    const vec4 *gpos = which ? (const vec4 *)ws.gpos64 : (const vec4 *)ws.gpos32;
-    const vec4 *spos = which ? (const vec4 *)ws.stage_pos64 : (const vec4 *)ws.stage_pos32;
-    const vec4 *mu = which ? (const vec4 *)c->mu64 : (const vec4 *)c->mu32;
-    k_cluster_tmu<real><<<ws.n_groups, GT, smem, s>>>(ws, gpos, spos, mu, k, c->acc, c->n_pad, s_run);
-    c->n_launches += 1;
-    TKHP_CUDA(c, cudaGetLastError());
-    return TKHP_OK;
-}
-
-int cluster_tmatvec(Ctx *c, cudaStream_t s) {
-    ClusterWs ws = get_ws(c);
-    return c->p.precision == TKHP_MIXED ? launch_tmu<float>(c, ws, s) : launch_tmu<double>(c, ws, s);
-}
-
-int cluster_field(Ctx *c, cudaStream_t s) {
-    // the permanent field runs once per solve: it walks the block-pair list (tiles.cu);
-    // run_field() has zeroed the accumulators
-    return tiles_field(c, s);
 }
 
 long long cluster_slots(Ctx *c) { return 8LL * c->h_state->n_cluster_entries; }

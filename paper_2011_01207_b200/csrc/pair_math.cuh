@@ -26,7 +26,8 @@ namespace tkhp {
 template <typename real>
 struct PairConsts {
     real beta;      // Ewald coefficient
-    real c1;        // 2/sqrt(pi) (0 when beta == 0 in FP64 mode: no exp term)
+    real c1;        // 2/sqrt(pi)
+    real c23;       // (2/3) c1
     real rc2;       // cutoff^2
     real box;       // box edge (PPI kernels)
     real inv_box;
@@ -62,33 +63,68 @@ __device__ __forceinline__ float erfcx_f32(float z) {
     return p;
 }
 
-// ---- MIXED: G_1..G_NK for an unmasked pair -------------------------------------------------
-template <int NK>
-__device__ __forceinline__ void radial_f32(float r2, float ww, const PairConsts<float> &k, float *G) {
-    const float rinv = fast_rsqrt(r2);
-    const float r = r2 * rinv;
-    const float rinv2 = rinv * rinv;
-    const float z = k.beta * r;
-    const float z2 = z * z;
-    const float ez = fast_ex2(z2 * -1.4426950408889634f);
-    const float g1 = fmaf(k.c1, z, erfcx_f32(z));      // erfcx(z) + c z
-    const float t = r * ww;
-    const float x = t * t * t;
-    const float et = fast_ex2(x * -1.4426950408889634f);
-    const float rinv3 = rinv2 * rinv;
-    G[0] = fmaf(ez, g1, -et) * rinv3;
+// ---- MIXED: G_1..G_NK for W unmasked pairs at once ------------------------------------------
+// Written stage by stage over W independent pairs so that the scheduler can interleave W
+// dependency chains (the Horner chain alone is 8 dependent FFMAs); W = 2 in the cluster kernels.
+// Scaled forms: R^3 G1 = ez g1 - et;  R^5 G2 / 3 = ez (g1 + (2c/3) z^3) - (1+x) et;
+// R^7 G3 / 15 = ez (g1 + (2c/3) z^3 + (4c/15) z^5) - (1 + x + 0.6 x^2) et.
+template <int NK, int W>
+__device__ __forceinline__ void radial_f32_w(const float (&r2)[W], const float (&ww)[W],
+                                             const PairConsts<float> &k, float (&G)[W][NK]) {
+    constexpr float c[TKHP_ERFCX_DEG + 1] = TKHP_ERFCX_COEFFS;
+    constexpr float NLOG2E = -1.4426950408889634f;
+    float rinv[W], r[W], z[W], u[W], p[W], z2[W], ez[W], t[W], x[W], et[W], g1[W], rinv2[W], rinv3[W];
+#pragma unroll
+    for (int i = 0; i < W; ++i) rinv[i] = fast_rsqrt(r2[i]);
+#pragma unroll
+    for (int i = 0; i < W; ++i) r[i] = r2[i] * rinv[i];
+#pragma unroll
+    for (int i = 0; i < W; ++i) z[i] = k.beta * r[i];
+#pragma unroll
+    for (int i = 0; i < W; ++i) u[i] = fast_rcp(fmaf(TKHP_ERFCX_P, z[i], 1.0f));
+#pragma unroll
+    for (int i = 0; i < W; ++i) { z2[i] = z[i] * z[i]; t[i] = r[i] * ww[i]; }
+#pragma unroll
+    for (int i = 0; i < W; ++i) { ez[i] = fast_ex2(z2[i] * NLOG2E); x[i] = t[i] * t[i] * t[i]; }
+#pragma unroll
+    for (int i = 0; i < W; ++i) { et[i] = fast_ex2(x[i] * NLOG2E); p[i] = c[TKHP_ERFCX_DEG]; }
+#pragma unroll
+    for (int d = TKHP_ERFCX_DEG - 1; d >= 0; --d) {
+#pragma unroll
+        for (int i = 0; i < W; ++i) p[i] = fmaf(p[i], u[i], c[d]);
+    }
+#pragma unroll
+    for (int i = 0; i < W; ++i) {
+        g1[i] = fmaf(k.c1, z[i], p[i]);                 // erfcx(z) + c z
+        rinv2[i] = rinv[i] * rinv[i];
+        rinv3[i] = rinv2[i] * rinv[i];
+        G[i][0] = fmaf(ez[i], g1[i], -et[i]) * rinv3[i];
+    }
     if (NK >= 2) {
-        const float cz3 = k.c1 * z * z2;               // c z^3
-        const float h2 = fmaf(2.0f, cz3, 3.0f * g1);   // 3 g1 + 2 c z^3
-        const float rinv5 = rinv3 * rinv2;
-        const float d5 = 3.0f * fmaf(x, et, et);       // 3 (1+x) e^-x
-        G[1] = fmaf(ez, h2, -d5) * rinv5;
-        if (NK >= 3) {
-            const float h3 = fmaf(4.0f * cz3, z2, 5.0f * h2);            // 5 h2 + 4 c z^5
-            const float d7 = 15.0f * fmaf(fmaf(0.6f, x, 1.0f) * x, et, et);  // 15 (1+x+0.6x^2) e^-x
-            G[2] = fmaf(ez, h3, -d7) * (rinv5 * rinv2);
+#pragma unroll
+        for (int i = 0; i < W; ++i) {
+            const float t5 = (k.c23 * z[i]) * z2[i];    // (2c/3) z^3
+            const float h2 = g1[i] + t5;
+            const float xet = x[i] * et[i];
+            const float xe = xet + et[i];               // (1+x) e^-x
+            const float r5 = (3.0f * rinv2[i]) * rinv3[i];
+            G[i][1] = fmaf(ez[i], h2, -xe) * r5;
+            if (NK >= 3) {
+                const float h3 = fmaf(0.4f * t5, z2[i], h2);
+                const float xe7 = fmaf(0.6f * x[i], xet, xe);   // (1 + x + 0.6 x^2) e^-x
+                G[i][2] = fmaf(ez[i], h3, -xe7) * ((5.0f * rinv2[i]) * r5);
+            }
         }
     }
+}
+
+template <int NK>
+__device__ __forceinline__ void radial_f32(float r2, float ww, const PairConsts<float> &k, float *G) {
+    const float r2a[1] = {r2}, wwa[1] = {ww};
+    float Ga[1][NK];
+    radial_f32_w<NK, 1>(r2a, wwa, k, Ga);
+#pragma unroll
+    for (int i = 0; i < NK; ++i) G[i] = Ga[0][i];
 }
 
 // ---- FP64: G_1..G_NK for an unmasked pair --------------------------------------------------
@@ -123,6 +159,17 @@ template <int NK>
 __device__ __forceinline__ void radial(float r2, float ww, const PairConsts<float> &k, float *G) {
     radial_f32<NK>(r2, ww, k, G);
 }
+template <int NK, int W>
+__device__ __forceinline__ void radial_w(const float (&r2)[W], const float (&ww)[W], const PairConsts<float> &k,
+                                         float (&G)[W][NK]) {
+    radial_f32_w<NK, W>(r2, ww, k, G);
+}
+template <int NK, int W>
+__device__ __forceinline__ void radial_w(const double (&r2)[W], const double (&ww)[W], const PairConsts<double> &k,
+                                         double (&G)[W][NK]) {
+#pragma unroll
+    for (int i = 0; i < W; ++i) radial_f64<NK>(r2[i], ww[i], k, G[i]);
+}
 template <int NK>
 __device__ __forceinline__ void radial(double r2, double ww, const PairConsts<double> &k, double *G) {
     radial_f64<NK>(r2, ww, k, G);
@@ -154,9 +201,10 @@ template <typename real>
 __device__ __forceinline__ void tmu_apply(real m1, real m2, real Rx, real Ry, real Rz, real mx, real my,
                                           real mz, real &ox, real &oy, real &oz) {
     const real c = m2 * (mx * Rx + my * Ry + mz * Rz);
-    ox += c * Rx - m1 * mx;
-    oy += c * Ry - m1 * my;
-    oz += c * Rz - m1 * mz;
+    const real n1 = -m1;
+    ox = fma(c, Rx, fma(n1, mx, ox));
+    oy = fma(c, Ry, fma(n1, my, oy));
+    oz = fma(c, Rz, fma(n1, mz, oz));
 }
 
 // ---- (F2) field at the point R away from a multipole (q, d, Q); sign = +1: R = r_i - r_j ----
@@ -171,10 +219,11 @@ __device__ __forceinline__ void field_apply(const real *G, real Rx, real Ry, rea
     const real tz = qxz * Rx + qyz * Ry + qzz * Rz;
     const real RTR = Rx * tx + Ry * ty + Rz * tz;
     const real rad = q * G[0] + G[1] * dR + (G[2] * (real)(1.0 / 3.0)) * RTR;
-    const real g23 = G[1] * (real)(2.0 / 3.0);
-    ex += rad * Rx - G[0] * dx - g23 * tx;
-    ey += rad * Ry - G[0] * dy - g23 * ty;
-    ez += rad * Rz - G[0] * dz - g23 * tz;
+    const real g23 = G[1] * (real)(-2.0 / 3.0);
+    const real n1 = -G[0];
+    ex = fma(rad, Rx, fma(n1, dx, fma(g23, tx, ex)));
+    ey = fma(rad, Ry, fma(n1, dy, fma(g23, ty, ey)));
+    ez = fma(rad, Rz, fma(n1, dz, fma(g23, tz, ez)));
 }
 
 }  // namespace tkhp

@@ -196,6 +196,7 @@ static PairConsts<real> make_consts(const tkhp_params &p) {
     PairConsts<real> k;
     k.beta = (real)p.ewald_beta;
     k.c1 = (real)(2.0 / SQRT_PI);
+    k.c23 = (real)(4.0 / (3.0 * SQRT_PI));
     k.rc2 = (real)(p.cutoff * p.cutoff);
     k.box = (real)(p.box > 0.0 ? p.box : 1.0);
     k.inv_box = (real)(p.box > 0.0 ? 1.0 / p.box : 0.0);
