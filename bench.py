@@ -2,7 +2,7 @@
 """bench.py -- headline benchmark of the real-space AMOEBA polarization hot path.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--config 0|1|2|3] [--precision mixed|fp64] [--list-mode auto|tiles|cluster]
+                    [--config 0|1|2|3] [--precision mixed|fp64] [--list-mode auto|tiles|cluster|atom]
 
 One STEP = one pass of the whole hot path over one synthetic system:
 neighbour-list build -> permanent field -> PCG solve to RMS 1e-6 -> polarization energy
@@ -52,7 +52,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3])
     ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
-    ap.add_argument("--list-mode", default="auto", choices=["auto", "tiles", "cluster"])
+    ap.add_argument("--list-mode", default="auto", choices=["auto", "tiles", "cluster", "atom"])
     ap.add_argument("--tol", type=float, default=1e-6)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -191,8 +191,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     sys_ = make_config(args.config)
     n = sys_.n_atoms
     precision = pk.TKHP_MIXED if args.precision == "mixed" else pk.TKHP_FP64
-    want_mode = {"auto": pk.TKHP_LIST_CLUSTER, "cluster": pk.TKHP_LIST_CLUSTER,
+    want_mode = {"auto": pk.TKHP_LIST_ATOM, "atom": pk.TKHP_LIST_ATOM, "cluster": pk.TKHP_LIST_CLUSTER,
                  "tiles": pk.TKHP_LIST_TILES}[args.list_mode]
+    mode_name = {pk.TKHP_LIST_TILES: "tiles", pk.TKHP_LIST_CLUSTER: "cluster", pk.TKHP_LIST_ATOM: "atom"}
     P = pk.Polarizer.for_system(sys_, precision=precision, list_mode=want_mode, device=local_rank)
     f64 = torch.float64
     d_pos = torch.as_tensor(sys_.pos, dtype=f64, device=dev)
@@ -262,7 +263,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     achieved = FLOPS_PER_PAIR_TMU * n_pair / (tmu_ms * 1e-3) / 1e12
     executed = FLOPS_PER_PAIR_TMU * n_slots / (tmu_ms * 1e-3) / 1e12
     roofline = {
-        "bound": "alu", "kernel": "T.mu pair kernel (%s list)" % ("cluster" if mode_in_use == pk.TKHP_LIST_CLUSTER else "tiles"),
+        "bound": "alu", "kernel": "T.mu pair kernel (%s list)" % mode_name[mode_in_use],
         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
         "traffic": None,
         "algorithmic_flops_per_launch": FLOPS_PER_PAIR_TMU * n_pair,
@@ -277,8 +278,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     try:
         traffic_file = ROOT / "profiles" / "traffic.json"
         if traffic_file.exists():
-            roofline["traffic"] = json.loads(traffic_file.read_text()).get(
-                "cluster" if mode_in_use == pk.TKHP_LIST_CLUSTER else "tiles")
+            roofline["traffic"] = json.loads(traffic_file.read_text()).get(mode_name[mode_in_use])
     except Exception:
         pass
 
@@ -346,7 +346,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "config": {"workload": WORKLOADS[args.config], "n_atoms": n, "box": sys_.box,
                    "cutoff": sys_.cutoff, "skin": sys_.skin, "ewald_beta": sys_.ewald_beta,
                    "tol": args.tol, "precision": args.precision,
-                   "list_mode": "cluster" if mode_in_use == pk.TKHP_LIST_CLUSTER else "tiles",
+                   "list_mode": mode_name[mode_in_use],
                    "parallelism": "replicas x%d" % world, "l2": "flushed between timed steps (256 MiB fill)"},
         "n_pair_within_cutoff": n_pair, "pcg_iterations": statistics.mean(iters),
         "pair_interactions_per_step": pairs_per_step, "energy_kcal_mol": energy, "final_rms": rms,

@@ -60,16 +60,20 @@ enum {
 /* which pair-list the compute kernels walk (both are built from the same 32-atom blocks) */
 enum {
     TKHP_LIST_TILES = 0,   /* one warp per 32x32 block pair of the block-pair list */
-    TKHP_LIST_CLUSTER = 1  /* filtered 8-atom-cluster -> atom lists, the paper's "list filtering"
+    TKHP_LIST_CLUSTER = 1, /* filtered 8-atom-cluster -> atom lists, the paper's "list filtering"
                                at finer granularity; falls back to TILES when the
                               box is too small for it (box/2 < cutoff + block extent) */
+    TKHP_LIST_ATOM = 2     /* the filtering carried to the end: one exact list per atom (every entry
+                              is a pair inside r_c for the positions of the build), stored
+                              lane-interleaved per 32-atom block; built from the CLUSTER lists.
+                              Falls back to CLUSTER (then TILES) when a capacity is exceeded */
 };
 
 typedef struct {
     int32_t n_atoms;     /* N >= 1 */
     int32_t precision;   /* TKHP_FP64 | TKHP_MIXED */
     int32_t device;      /* CUDA device ordinal */
-    int32_t list_mode;   /* TKHP_LIST_TILES | TKHP_LIST_CLUSTER */
+    int32_t list_mode;   /* TKHP_LIST_TILES | TKHP_LIST_CLUSTER | TKHP_LIST_ATOM */
     double box;          /* cubic box edge L; <= 0: open boundary, no images (tests) */
     double cutoff;       /* r_c: a pair contributes iff R^2 <= r_c^2 */
     double skin;         /* list buffer: block pairs kept by box distance <= r_c + skin */
@@ -77,6 +81,8 @@ typedef struct {
     double thole_a;      /* Thole width a (0.39 for AMOEBA water) */
     int32_t max_tiles_per_block; /* capacity of the block-pair list per block; 0 = automatic */
     int32_t max_nbrs_per_cluster; /* capacity of a cluster's atom list; 0 = automatic */
+    int32_t max_nbrs_per_atom;   /* ATOM mode: capacity of one atom's list incl. padding; 0 = automatic */
+    int32_t reserved;            /* must be 0 */
 } tkhp_params;
 
 /* Bytes of device workspace tkhp_create() needs for these parameters.  Host, pure. */
@@ -120,8 +126,9 @@ int tkhp_nblist_view(tkhp_ctx *ctx, int32_t *n_blocks, int64_t *n_pairs,
  *                          the "useful pair interactions" of one field / T.mu evaluation
  *   n_slots_evaluated      lane-slots the compute kernels of the active list mode walk
  *                          per evaluation (tiles: 1024 per off-diagonal tile, 992 per
- *                          diagonal tile; cluster: 8 x list length summed over clusters)
- *   list_mode_in_use       TKHP_LIST_TILES or TKHP_LIST_CLUSTER after any fallback   */
+ *                          diagonal tile; cluster: 8 x list length summed over clusters;
+ *                          atom: 32 x padded list length summed over blocks)
+ *   list_mode_in_use       TKHP_LIST_TILES, _CLUSTER or _ATOM after any fallback     */
 int tkhp_nblist_stats(tkhp_ctx *ctx, int64_t *n_pairs_within_cutoff, int64_t *n_slots_evaluated,
                       int32_t *list_mode_in_use, void *stream);
 

@@ -9,7 +9,7 @@ no CPU fallback: importing works without a GPU (so the build can be checked),
 but creating a context without a CUDA device raises, and a missing
 ``libtkhp.so`` raises at import of :mod:`paper_2011_01207_b200.binding`.
 """
-from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_LIST_TILES, TKHP_LIST_CLUSTER,
+from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM,
                       TkhpError, TkhpParams, Polarizer, lib, lib_path,
                       tkhp_workspace_bytes, tkhp_create, tkhp_destroy, tkhp_last_error,
                       tkhp_nblist_build, tkhp_nblist_view, tkhp_nblist_stats,
@@ -18,7 +18,7 @@ from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_LIST_TILES, TKHP_LIST_CLUSTER,
                       tkhp_fma_peak, tkhp_profile_reset, tkhp_profile_read, EXPORTED_SYMBOLS)
 
 __all__ = [
-    "TKHP_FP64", "TKHP_MIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TkhpError",
+    "TKHP_FP64", "TKHP_MIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TKHP_LIST_ATOM", "TkhpError",
     "TkhpParams", "Polarizer", "lib", "lib_path", "tkhp_workspace_bytes", "tkhp_create",
     "tkhp_destroy", "tkhp_last_error", "tkhp_nblist_build", "tkhp_nblist_view",
     "tkhp_nblist_stats", "tkhp_perm_field", "tkhp_tmatvec", "tkhp_polar_solve",

@@ -10,7 +10,7 @@ TKHP_OK = 0
 TKHP_EINVAL, TKHP_ECUDA, TKHP_ECUTOFF, TKHP_ENOLIST = -1, -2, -3, -4
 TKHP_ENOCONV, TKHP_ECAPACITY, TKHP_ENONFINITE = -5, -6, -7
 TKHP_FP64, TKHP_MIXED = 0, 1
-TKHP_LIST_TILES, TKHP_LIST_CLUSTER = 0, 1
+TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM = 0, 1, 2
 
 _ERR_NAMES = {-1: "TKHP_EINVAL", -2: "TKHP_ECUDA", -3: "TKHP_ECUTOFF", -4: "TKHP_ENOLIST",
               -5: "TKHP_ENOCONV", -6: "TKHP_ECAPACITY", -7: "TKHP_ENONFINITE"}
@@ -34,7 +34,8 @@ class TkhpParams(Structure):
     _fields_ = [("n_atoms", c_int32), ("precision", c_int32), ("device", c_int32),
                 ("list_mode", c_int32), ("box", c_double), ("cutoff", c_double),
                 ("skin", c_double), ("ewald_beta", c_double), ("thole_a", c_double),
-                ("max_tiles_per_block", c_int32), ("max_nbrs_per_cluster", c_int32)]
+                ("max_tiles_per_block", c_int32), ("max_nbrs_per_cluster", c_int32),
+                ("max_nbrs_per_atom", c_int32), ("reserved", c_int32)]
 
 
 def lib_path() -> Path:
@@ -233,14 +234,15 @@ class Polarizer:
 
     def __init__(self, n_atoms, box, cutoff=7.0, skin=2.0, ewald_beta=0.5446, thole_a=0.39,
                  precision=TKHP_MIXED, list_mode=TKHP_LIST_TILES, device=0,
-                 max_tiles_per_block=0, max_nbrs_per_cluster=0):
+                 max_tiles_per_block=0, max_nbrs_per_cluster=0, max_nbrs_per_atom=0):
         import torch
         if not torch.cuda.is_available():
             raise TkhpError(TKHP_ECUDA, "no CUDA device: libtkhp has no CPU fallback")
         self.torch = torch
         self.device = torch.device("cuda", device)
         self.params = TkhpParams(n_atoms, precision, device, list_mode, box, cutoff, skin,
-                                 ewald_beta, thole_a, max_tiles_per_block, max_nbrs_per_cluster)
+                                 ewald_beta, thole_a, max_tiles_per_block, max_nbrs_per_cluster,
+                                 max_nbrs_per_atom, 0)
         self.n = n_atoms
         nbytes = tkhp_workspace_bytes(self.params)
         with torch.cuda.device(self.device):

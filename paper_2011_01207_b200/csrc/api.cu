@@ -19,7 +19,7 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
     if (!p) { snprintf(err, n, "params is NULL"); return TKHP_EINVAL; }
     if (p->n_atoms < 1) { snprintf(err, n, "n_atoms must be >= 1"); return TKHP_EINVAL; }
     if (p->precision != TKHP_FP64 && p->precision != TKHP_MIXED) { snprintf(err, n, "bad precision"); return TKHP_EINVAL; }
-    if (p->list_mode != TKHP_LIST_TILES && p->list_mode != TKHP_LIST_CLUSTER) { snprintf(err, n, "bad list_mode"); return TKHP_EINVAL; }
+    if (p->list_mode != TKHP_LIST_TILES && p->list_mode != TKHP_LIST_CLUSTER && p->list_mode != TKHP_LIST_ATOM) { snprintf(err, n, "bad list_mode"); return TKHP_EINVAL; }
     if (!(p->cutoff > 0.0) || !(p->skin >= 0.0) || !isfinite(p->cutoff) || !isfinite(p->skin)) { snprintf(err, n, "cutoff must be > 0 and skin >= 0"); return TKHP_EINVAL; }
     if (!(p->ewald_beta >= 0.0) || !isfinite(p->ewald_beta)) { snprintf(err, n, "ewald_beta must be >= 0"); return TKHP_EINVAL; }
     if (!(p->thole_a > 0.0) || !isfinite(p->thole_a)) { snprintf(err, n, "thole_a must be > 0"); return TKHP_EINVAL; }
@@ -33,7 +33,7 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
         return TKHP_EINVAL;
     }
     if (p->precision == TKHP_MIXED && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }
-    if (p->max_tiles_per_block < 0 || p->max_nbrs_per_cluster < 0) { snprintf(err, n, "negative capacity"); return TKHP_EINVAL; }
+    if (p->max_tiles_per_block < 0 || p->max_nbrs_per_cluster < 0 || p->max_nbrs_per_atom < 0) { snprintf(err, n, "negative capacity"); return TKHP_EINVAL; }
     return TKHP_OK;
 }
 
@@ -136,7 +136,9 @@ int ensure_header(Ctx *c, cudaStream_t s) {
         TKHP_CUDA(c, cudaStreamSynchronize(s));
         c->header_valid = true;
         c->n_tiles_host = c->h_state->n_tiles;
-        c->list_mode_in_use = (c->p.list_mode == TKHP_LIST_CLUSTER && !c->h_state->cluster_bad) ? TKHP_LIST_CLUSTER : TKHP_LIST_TILES;
+        c->list_mode_in_use = TKHP_LIST_TILES;
+        if (c->p.list_mode != TKHP_LIST_TILES && !c->h_state->cluster_bad)
+            c->list_mode_in_use = (c->p.list_mode == TKHP_LIST_ATOM && !c->h_state->atom_bad) ? TKHP_LIST_ATOM : TKHP_LIST_CLUSTER;
     }
     const DeviceState &h = *c->h_state;
     if (h.err_nonfinite) return set_err(c, TKHP_ENONFINITE, "non-finite position passed to tkhp_nblist_build%s");
@@ -239,9 +241,13 @@ int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polari
     if (rc) return rc;
     c->built = true;
     c->list_mode_in_use = TKHP_LIST_TILES;
-    if (c->p.list_mode == TKHP_LIST_CLUSTER) {
+    if (c->p.list_mode != TKHP_LIST_TILES) {
         rc = cluster_build(c, s);
         if (rc) return rc;
+        if (c->p.list_mode == TKHP_LIST_ATOM) {
+            rc = atom_build(c, s);
+            if (rc) return rc;
+        }
     }
     toc(c, 0, s);
     return TKHP_OK;
@@ -277,7 +283,9 @@ int tkhp_nblist_stats(tkhp_ctx *ctx, int64_t *n_pairs_within_cutoff, int64_t *n_
         *n_pairs_within_cutoff = v;
     }
     if (n_slots_evaluated) {
-        if (c->list_mode_in_use == TKHP_LIST_CLUSTER) {
+        if (c->list_mode_in_use == TKHP_LIST_ATOM) {
+            *n_slots_evaluated = atom_slots(c);
+        } else if (c->list_mode_in_use == TKHP_LIST_CLUSTER) {
             *n_slots_evaluated = cluster_slots(c);
         } else {
             const long long diag = c->n_blocks;

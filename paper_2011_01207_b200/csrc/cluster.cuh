@@ -36,6 +36,20 @@ constexpr int CB_CAP = 1024;          // candidate blocks per group
 constexpr int RESIDENT = 3;           // CTAs per SM the group count is rounded to
 constexpr int B200_SMS = 148;
 constexpr float GUARD = 0.01f;        // list radius = r_c + GUARD (FP32 build arithmetic is safe)
+constexpr int NCH_MAX = 16;           // ATOM mode: max staging chunks per group
+constexpr int ATOM_SMEM = 56 * 1024;  // ATOM mode: shared memory of the T.mu kernel per CTA (4 CTAs / SM)
+
+// ATOM mode chunking of a group's staged atoms: the same function on the host (launch geometry)
+// and on the device (list construction), from the largest staged-atom count of any group.
+__host__ __device__ inline void atom_chunking(int max_stage, bool f64, int *n_chunks, int *s_chunk) {
+    const int s_max = (ATOM_SMEM / (f64 ? 64 : 32) - 1) & ~31;   // records of pos + mu
+    if (max_stage < 1) max_stage = 1;
+    const int n = (max_stage + s_max - 1) / s_max;
+    int s = (((max_stage + n - 1) / n) + 31) & ~31;
+    if (s > s_max) s = s_max;
+    *n_chunks = n;
+    *s_chunk = s;
+}
 
 struct ClusterWs {
     int n_groups, s_cap, l_cap;
@@ -49,6 +63,12 @@ struct ClusterWs {
     uint32_t *stage_mask;             // n_groups * s_cap: which clusters of the group list the atom
     uint16_t *entries;                // (n_pad/8) * l_cap
     int32_t *oct_len;                 // n_pad/8: padded list length (equal within a warp)
+    // ATOM list mode (atom_pairs.cu): per-atom lists, one u16 BYTE OFFSET into the staged chunk per
+    // entry, laid out per block as [entry/4][lane][entry%4] so that a lane reads 4 entries with one
+    // coalesced 8-byte load; every chunk's list is padded to the longest lane of the warp.
+    int a_cap;                        // entries per lane and block (multiple of 4)
+    uint16_t *alist;                  // n_blocks * a_cap * 32
+    int32_t *arow;                    // n_blocks * (NCH_MAX + 1): first entry of each chunk's list
 };
 
 inline int choose_groups(int n_blocks) {
@@ -101,6 +121,23 @@ inline size_t carve_cluster(const tkhp_params *p, int n_blocks, void *base, Clus
     ws.stage_mask = w.take<uint32_t>(gs);
     ws.entries = w.take<uint16_t>((n_pad / CLUSTER) * ws.l_cap);
     ws.oct_len = w.take<int32_t>(n_pad / CLUSTER);
+    ws.a_cap = 0; ws.alist = nullptr; ws.arow = nullptr;
+    if (p->list_mode == TKHP_LIST_ATOM) {
+        long long a;
+        if (p->max_nbrs_per_atom > 0) {
+            a = p->max_nbrs_per_atom;
+        } else if (p->box > 0.0) {
+            const double rho = p->n_atoms / (p->box * p->box * p->box);
+            const double r = p->cutoff + 0.05;
+            a = (long long)(1.6 * 4.18879 * r * r * r * rho) + 48;
+        } else {
+            a = 1024;
+        }
+        if (a > (long long)n_pad + 8 * NCH_MAX) a = (long long)n_pad + 8 * NCH_MAX;
+        ws.a_cap = (int)((a + 7) & ~7LL);
+        ws.alist = w.take<uint16_t>((size_t)n_blocks * ws.a_cap * 32);
+        ws.arow = w.take<int32_t>((size_t)n_blocks * (NCH_MAX + 1));
+    }
     w.take<char>(256);
     if (out) *out = ws;
     return w.off;

@@ -250,7 +250,7 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
 }
 
 size_t cluster_workspace_bytes(const tkhp_params *p, int n_blocks) {
-    if (p->list_mode != TKHP_LIST_CLUSTER) return 0;
+    if (p->list_mode == TKHP_LIST_TILES) return 0;
     return carve_cluster(p, n_blocks, nullptr, nullptr);
 }
 

@@ -42,6 +42,9 @@ struct DeviceState {
     long long n_diag_tiles;
     long long n_cluster_entries;        // total entries of all cluster lists (CLUSTER mode)
     long long n_pairs_within_cutoff;    // statistics (tkhp_nblist_stats)
+    long long n_atom_entries;           // ATOM mode: padded per-lane list entries summed over blocks
+    int atom_bad;                       // 1: ATOM lists unusable (capacity / too many chunks): CLUSTER is used
+    int pad1;
     // PCG scalars
     double rz, pq, rr, gamma, delta;
     int converged;
@@ -158,6 +161,10 @@ int cluster_build(Ctx *c, cudaStream_t s);
 int cluster_tmatvec(Ctx *c, cudaStream_t s);
 int cluster_field(Ctx *c, cudaStream_t s);
 long long cluster_slots(Ctx *c);
+int atom_build(Ctx *c, cudaStream_t s);
+int atom_tmatvec(Ctx *c, cudaStream_t s);
+int atom_field(Ctx *c, cudaStream_t s);
+long long atom_slots(Ctx *c);
 
 int run_tmatvec(Ctx *c, cudaStream_t s);            // dispatch on list mode; zeroes acc first
 int run_field(Ctx *c, cudaStream_t s);

@@ -302,17 +302,22 @@ static inline void prof_end(Ctx *c, int which, cudaStream_t s) {
 
 int run_tmatvec(Ctx *c, cudaStream_t s) {
     // the tile kernel accumulates with atomics into zeroed accumulators; the cluster kernel stores
-    if (c->list_mode_in_use != TKHP_LIST_CLUSTER)
+    if (c->list_mode_in_use == TKHP_LIST_TILES)
         TKHP_CUDA(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 3 * (size_t)c->n_pad, s));
     const bool rec = prof_begin(c, 0, s);
-    int rc = c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_tmatvec(c, s) : tiles_tmatvec(c, s);
+    int rc = c->list_mode_in_use == TKHP_LIST_ATOM      ? atom_tmatvec(c, s)
+             : c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_tmatvec(c, s)
+                                                        : tiles_tmatvec(c, s);
     if (rec) prof_end(c, 0, s);
     return rc;
 }
 int run_field(Ctx *c, cudaStream_t s) {
-    TKHP_CUDA(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 3 * (size_t)c->n_pad, s));
+    if (c->list_mode_in_use == TKHP_LIST_TILES)
+        TKHP_CUDA(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 3 * (size_t)c->n_pad, s));
     const bool rec = prof_begin(c, 1, s);
-    int rc = c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_field(c, s) : tiles_field(c, s);
+    int rc = c->list_mode_in_use == TKHP_LIST_ATOM      ? atom_field(c, s)
+             : c->list_mode_in_use == TKHP_LIST_CLUSTER ? cluster_field(c, s)
+                                                        : tiles_field(c, s);
     if (rec) prof_end(c, 1, s);
     return rc;
 }

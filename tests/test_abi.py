@@ -36,11 +36,22 @@ def test_binding_lists_every_symbol(built_lib):
         assert callable(getattr(pk, name)), name
 
 
-def test_params_struct_layout_matches_header(built_lib):
+def test_params_struct_layout_matches_header(built_lib, tmp_path):
+    """sizeof/offsetof of tkhp_params as gcc sees include/tkhp.h == the ctypes mirror."""
+    import subprocess
     import paper_2011_01207_b200 as pk
-    # 4 int32, 5 double, 2 int32  -> 16 + 40 + 8 = 64 bytes, doubles 8-aligned
-    assert ctypes.sizeof(pk.TkhpParams) == 64
-    assert pk.TkhpParams.box.offset == 16 and pk.TkhpParams.max_tiles_per_block.offset == 56
+    names = [f[0] for f in pk.TkhpParams._fields_]
+    src = tmp_path / "layout.c"
+    body = "".join(f'    printf("{n} %zu\\n", offsetof(tkhp_params, {n}));\n' for n in names)
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "tkhp.h"\nint main(void) {\n'
+                   '    printf("sizeof %zu\\n", sizeof(tkhp_params));\n' + body + "    return 0;\n}\n")
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-I", str(ROOT / "include"), str(src), "-o", str(exe)], check=True)
+    out = dict(line.split() for line in subprocess.run([str(exe)], check=True, capture_output=True,
+                                                       text=True).stdout.splitlines())
+    assert int(out["sizeof"]) == ctypes.sizeof(pk.TkhpParams) == 72
+    for n in names:
+        assert int(out[n]) == getattr(pk.TkhpParams, n).offset, n
 
 
 def test_host_side_parameter_checks(built_lib):

@@ -34,13 +34,13 @@ def _rows(s, perm, n_rand=512, n_blocks=4, seed=0):
     return np.array(sorted(rows), dtype=np.int64)
 
 
-@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster", "atom"])
 @pytest.mark.parametrize("precision", ["fp64", "mixed"])
 def test_cfg1_full_parity(cfg1, precision, list_mode):
     import paper_2011_01207_b200 as pk
     s = cfg1
     P = pk.Polarizer.for_system(s, precision=pk.TKHP_FP64 if precision == "fp64" else pk.TKHP_MIXED,
-                                list_mode=pk.TKHP_LIST_TILES if list_mode == "tiles" else pk.TKHP_LIST_CLUSTER)
+                                list_mode={"tiles": pk.TKHP_LIST_TILES, "cluster": pk.TKHP_LIST_CLUSTER, "atom": pk.TKHP_LIST_ATOM}[list_mode])
     P.nblist_build(s.pos, s.polarizability, s.group_id)
     perm, pairs = P.nblist_view()
     oracle.check_perm(perm, s.pos, s.box)
@@ -66,15 +66,15 @@ def test_cfg1_full_parity(cfg1, precision, list_mode):
     P.close()
 
 
-@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster", "atom"])
 def test_cfg2_sampled_rows_mixed(cfg2, list_mode):
     """Config 2 (98,304 atoms, 15% solutes), MIXED: the configuration bench.py times."""
     import paper_2011_01207_b200 as pk
     s = cfg2
     P = pk.Polarizer.for_system(s, precision=pk.TKHP_MIXED,
-                                list_mode=pk.TKHP_LIST_TILES if list_mode == "tiles" else pk.TKHP_LIST_CLUSTER)
+                                list_mode={"tiles": pk.TKHP_LIST_TILES, "cluster": pk.TKHP_LIST_CLUSTER, "atom": pk.TKHP_LIST_ATOM}[list_mode])
     P.nblist_build(s.pos, s.polarizability, s.group_id)
-    assert P.nblist_stats(count_pairs=False)[2] == (pk.TKHP_LIST_CLUSTER if list_mode == "cluster" else pk.TKHP_LIST_TILES)
+    assert P.nblist_stats(count_pairs=False)[2] == {"tiles": pk.TKHP_LIST_TILES, "cluster": pk.TKHP_LIST_CLUSTER, "atom": pk.TKHP_LIST_ATOM}[list_mode]
     P.nblist_build(s.pos, s.polarizability, s.group_id)
     perm, pairs = P.nblist_view()
     oracle.check_perm(perm, s.pos, s.box)

@@ -26,7 +26,7 @@ def _polarizer(s, precision, list_mode="tiles"):
     pk = _pk()
     P = pk.Polarizer.for_system(
         s, precision=pk.TKHP_FP64 if precision == "fp64" else pk.TKHP_MIXED,
-        list_mode=pk.TKHP_LIST_TILES if list_mode == "tiles" else pk.TKHP_LIST_CLUSTER)
+        list_mode={"tiles": pk.TKHP_LIST_TILES, "cluster": pk.TKHP_LIST_CLUSTER, "atom": pk.TKHP_LIST_ATOM}[list_mode])
     P.nblist_build(s.pos, s.polarizability, s.group_id)
     return P
 
@@ -82,7 +82,7 @@ def test_nblist_is_deterministic_and_rebuildable():
 
 
 # ------------------------------------------------------------------ T.mu and field
-@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster", "atom"])
 @pytest.mark.parametrize("precision", ["fp64", "mixed"])
 def test_tmatvec_matches_oracle(system, precision, list_mode):
     s = system
@@ -95,7 +95,7 @@ def test_tmatvec_matches_oracle(system, precision, list_mode):
     P.close()
 
 
-@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster", "atom"])
 @pytest.mark.parametrize("precision", ["fp64", "mixed"])
 def test_perm_field_matches_oracle(system, precision, list_mode):
     s = system
@@ -130,6 +130,35 @@ def test_cluster_mode_is_used_and_deterministic():
     small.close()
 
 
+def test_atom_mode_lists_are_exact_and_deterministic():
+    """ATOM lists: active on a big enough box, every list entry is a pair inside r_c (executed
+    slots = ordered useful pairs + warp padding only), results bit-identical run to run, and the
+    capacity fallback lands on CLUSTER with the same answers."""
+    pk = _pk()
+    s = SYSTEMS["water_6000"]()
+    P = _polarizer(s, "mixed", "atom")
+    n_pair, n_slots, mode = P.nblist_stats()
+    assert mode == pk.TKHP_LIST_ATOM and n_pair == oracle.count_pairs(s)
+    assert 2 * n_pair <= n_slots <= 3 * n_pair          # padding to the longest lane of a warp only
+    rng = np.random.default_rng(3)
+    mu = rng.standard_normal((s.n_atoms, 3))
+    a = P.tmatvec(mu).cpu().numpy()
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    b = P.tmatvec(mu).cpu().numpy()
+    assert np.array_equal(a, b)
+    P.close()
+    tight = pk.Polarizer.for_system(s, precision=pk.TKHP_MIXED, list_mode=pk.TKHP_LIST_ATOM,
+                                    max_nbrs_per_atom=64)       # ~144 neighbours needed
+    tight.nblist_build(s.pos, s.polarizability, s.group_id)
+    assert tight.nblist_stats(count_pairs=False)[2] == pk.TKHP_LIST_CLUSTER
+    c = tight.tmatvec(mu).cpu().numpy()
+    assert _rel_l2(c, a) <= 1e-6
+    tight.close()
+    small = _polarizer(make_config(0), "mixed", "atom")
+    assert small.nblist_stats()[2] == pk.TKHP_LIST_TILES
+    small.close()
+
+
 def test_tmatvec_symmetry_on_gpu():
     """nu.T mu == mu.T nu for the GPU operator as well (FP64 mode)."""
     import torch
@@ -144,7 +173,7 @@ def test_tmatvec_symmetry_on_gpu():
 
 
 # ------------------------------------------------------------------ solve and energy
-@pytest.mark.parametrize("list_mode", ["tiles", "cluster"])
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster", "atom"])
 @pytest.mark.parametrize("precision", ["fp64", "mixed"])
 @pytest.mark.parametrize("name", ["cfg0", "n65_periodic", "water_1536_solutes", "water_6000"])
 def test_solve_and_energy_match_oracle(name, precision, list_mode):
