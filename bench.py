@@ -171,6 +171,7 @@ def run_reference(args, rank: int, world: int):
 def run_ours(args, rank: int, world: int, local_rank: int):
     import torch
     import paper_2011_01207_b200 as pk
+    from paper_2011_01207_b200 import replicas
     from synth_inputs import make_config
 
     if not torch.cuda.is_available():
@@ -247,14 +248,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     phase_ms = P.timings()
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = sum(step_ms)
-    if dist is not None:
-        t = torch.tensor([total_ms, wall_s], dtype=f64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, wall_s = float(t[0]), float(t[1])
+    total_ms, wall_s = replicas.max_over_ranks([total_ms, wall_s], dist, dev)
+    if not replicas.replicas_agree(statistics.mean(iters), energy, dist, dev):
+        raise SystemExit("bench.py: replicas disagree on iteration count or energy")
     ms_per_step = total_ms / args.steps
     n_matvec = statistics.mean(iters) + 1
     pairs_per_step = n_pair * (1 + n_matvec)
-    value = world * pairs_per_step / (ms_per_step * 1e-3)
+    value = replicas.aggregate_throughput(pairs_per_step, world, ms_per_step)
 
     # ---- dominant kernel roofline (T.mu pair kernel), measured live with CUDA events
     tmu_ms = prof_tot["tmatvec_ms"] / max(prof_tot["n_tmatvec"], 1)
@@ -307,12 +307,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             e2e_iters.append(it2)
         barrier()
         tot = sum(e2e_ms)
-        if dist is not None:
-            t = torch.tensor([tot], dtype=f64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            tot = float(t[0])
+        (tot,) = replicas.max_over_ranks([tot], dist, dev)
         e2e_step = tot / args.steps
-        e2e = {"value": world * n_pair * (2 + statistics.mean(e2e_iters)) / (e2e_step * 1e-3), "unit": UNIT,
+        e2e = {"value": replicas.aggregate_throughput(n_pair * (2 + statistics.mean(e2e_iters)), world, e2e_step),
+               "unit": UNIT,
                "ms_per_step": e2e_step,
                "h2d_bytes_per_step": n * (24 + 8 + 4 + 8 + 24 + 48),
                "d2h_bytes_per_step": n * 24 + 8}
@@ -365,8 +363,8 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if world == 1 and args.gpus > 1 and args.impl == "ours":
         # plain `python bench.py --gpus N`: re-launch under torchrun, one rank per GPU
-        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
-               "--master-addr", "127.0.0.1", "--master-port", "29531", str(Path(__file__).resolve())] + sys.argv[1:]
+        from paper_2011_01207_b200 import replicas
+        cmd = replicas.torchrun_command(sys.executable, str(Path(__file__).resolve()), args.gpus, sys.argv[1:])
         raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args, rank, world)
