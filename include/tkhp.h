@@ -82,7 +82,9 @@ typedef struct {
     int32_t max_tiles_per_block; /* capacity of the block-pair list per block; 0 = automatic */
     int32_t max_nbrs_per_cluster; /* capacity of a cluster's atom list; 0 = automatic */
     int32_t max_nbrs_per_atom;   /* ATOM mode: capacity of one atom's list incl. padding; 0 = automatic */
-    int32_t reserved;            /* must be 0 */
+    int32_t max_stage_per_chunk; /* ATOM mode: staged atoms per shared-memory chunk (multiple of 32);
+                                    0 = automatic (what fits the kernel's shared memory); tests use a
+                                    small value to exercise the multi-chunk path */
 } tkhp_params;
 
 /* Bytes of device workspace tkhp_create() needs for these parameters.  Host, pure. */

@@ -35,7 +35,7 @@ class TkhpParams(Structure):
                 ("list_mode", c_int32), ("box", c_double), ("cutoff", c_double),
                 ("skin", c_double), ("ewald_beta", c_double), ("thole_a", c_double),
                 ("max_tiles_per_block", c_int32), ("max_nbrs_per_cluster", c_int32),
-                ("max_nbrs_per_atom", c_int32), ("reserved", c_int32)]
+                ("max_nbrs_per_atom", c_int32), ("max_stage_per_chunk", c_int32)]
 
 
 def lib_path() -> Path:
@@ -234,7 +234,8 @@ class Polarizer:
 
     def __init__(self, n_atoms, box, cutoff=7.0, skin=2.0, ewald_beta=0.5446, thole_a=0.39,
                  precision=TKHP_MIXED, list_mode=TKHP_LIST_TILES, device=0,
-                 max_tiles_per_block=0, max_nbrs_per_cluster=0, max_nbrs_per_atom=0):
+                 max_tiles_per_block=0, max_nbrs_per_cluster=0, max_nbrs_per_atom=0,
+                 max_stage_per_chunk=0):
         import torch
         if not torch.cuda.is_available():
             raise TkhpError(TKHP_ECUDA, "no CUDA device: libtkhp has no CPU fallback")
@@ -242,7 +243,7 @@ class Polarizer:
         self.device = torch.device("cuda", device)
         self.params = TkhpParams(n_atoms, precision, device, list_mode, box, cutoff, skin,
                                  ewald_beta, thole_a, max_tiles_per_block, max_nbrs_per_cluster,
-                                 max_nbrs_per_atom, 0)
+                                 max_nbrs_per_atom, max_stage_per_chunk)
         self.n = n_atoms
         nbytes = tkhp_workspace_bytes(self.params)
         with torch.cuda.device(self.device):

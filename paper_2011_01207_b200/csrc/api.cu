@@ -34,6 +34,7 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
     }
     if (p->precision == TKHP_MIXED && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }
     if (p->max_tiles_per_block < 0 || p->max_nbrs_per_cluster < 0 || p->max_nbrs_per_atom < 0) { snprintf(err, n, "negative capacity"); return TKHP_EINVAL; }
+    if (p->max_stage_per_chunk < 0 || (p->max_stage_per_chunk & 31)) { snprintf(err, n, "max_stage_per_chunk must be a non-negative multiple of 32"); return TKHP_EINVAL; }
     return TKHP_OK;
 }
 
@@ -112,7 +113,8 @@ static size_t carve(Ctx *c, const tkhp_params *p, void *base) {
     o->vr = w.take<double>(3 * n_pad);
     o->vp = w.take<double>(3 * n_pad);
     o->vq = w.take<double>(3 * n_pad);
-    o->partials = w.take<double>(8 * MAX_PARTIALS);
+    o->part_cap = n_blocks + MAX_PARTIALS;
+    o->partials = w.take<double>(6 * (size_t)o->part_cap);
     // staging for the host-buffer entry
     o->h_pos = w.take<double>(3 * n);
     o->h_alpha = w.take<double>(n);
@@ -193,7 +195,13 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, params->device) != cudaSuccess) { delete c; return TKHP_ECUDA; }
     c->sm_count = prop.multiProcessorCount;
-    if (cudaMallocHost(&c->h_scalars, 8 * sizeof(double)) != cudaSuccess ||
+    c->spec_iter = -1;
+    c->fuse_q = false;
+    c->n_noop_launches = 0;
+    c->h_ring = c->d_ring = nullptr;
+    if (cudaHostAlloc(&c->h_ring, RING * sizeof(double), cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostGetDevicePointer(&c->d_ring, c->h_ring, 0) != cudaSuccess ||
+        cudaMallocHost(&c->h_scalars, 8 * sizeof(double)) != cudaSuccess ||
         cudaMallocHost(&c->h_state, sizeof(DeviceState)) != cudaSuccess) {
         snprintf(g_create_err, sizeof(g_create_err), "cudaMallocHost failed");
         delete c;
@@ -219,6 +227,7 @@ int tkhp_destroy(tkhp_ctx *ctx) {
     for (int i = 0; i < 10; ++i) cudaEventDestroy(c->ev[i]);
     for (int w = 0; w < 2; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventDestroy(c->prof_ev[w][i]);
+    cudaFreeHost(c->h_ring);
     cudaFreeHost(c->h_scalars);
     cudaFreeHost(c->h_state);
     delete c;
@@ -383,6 +392,7 @@ int tkhp_profile_reset(tkhp_ctx *ctx, int32_t enable_kernel_events) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     c->n_launches = 0;
+    c->n_noop_launches = 0;
     c->prof = enable_kernel_events != 0;
     c->prof_n[0] = c->prof_n[1] = 0;
     return TKHP_OK;
@@ -392,10 +402,12 @@ int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmat
                       double *tmatvec_kernel_ms, int32_t *n_field_kernels, double *field_kernel_ms) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
-    if (n_kernel_launches) *n_kernel_launches = c->n_launches;
+    if (n_kernel_launches) *n_kernel_launches = c->n_launches - c->n_noop_launches;
     double tot[2] = {0.0, 0.0};
+    int cnt[2] = {0, 0};
     for (int w = 0; w < 2; ++w) {
         for (int i = 0; i < c->prof_n[w]; ++i) {
+            if (c->prof_skip[w][i]) continue;
             float t = 0.f;
             if (cudaEventSynchronize(c->prof_ev[w][2 * i + 1]) != cudaSuccess ||
                 cudaEventElapsedTime(&t, c->prof_ev[w][2 * i], c->prof_ev[w][2 * i + 1]) != cudaSuccess) {
@@ -403,11 +415,12 @@ int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmat
                 return set_err(c, TKHP_ECUDA, "profile events not complete%s");
             }
             tot[w] += t;
+            cnt[w]++;
         }
     }
-    if (n_tmatvec_kernels) *n_tmatvec_kernels = c->prof_n[0];
+    if (n_tmatvec_kernels) *n_tmatvec_kernels = cnt[0];
     if (tmatvec_kernel_ms) *tmatvec_kernel_ms = tot[0];
-    if (n_field_kernels) *n_field_kernels = c->prof_n[1];
+    if (n_field_kernels) *n_field_kernels = cnt[1];
     if (field_kernel_ms) *field_kernel_ms = tot[1];
     return TKHP_OK;
 }

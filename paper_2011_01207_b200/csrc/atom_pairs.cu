@@ -22,10 +22,24 @@
 // The lists are built from the CLUSTER lists (the 8-atom-cluster list is the candidate set of
 // each of its atoms): k_atom_lists below.
 #include "cluster.cuh"
+#include "reduce.cuh"
 
 namespace tkhp {
 
 constexpr int MODE_TMU = 0, MODE_FIELD = 1;
+static_assert(GT == RED_THREADS, "the fused PCG epilogue uses the 256-thread block reductions");
+
+// PCG fusion (MODE_TMU): the lane that owns atom i holds (T p)_i when the
+// list is exhausted, so q_i = p_i/alpha_i - (T p)_i - self p_i and the block's share of p.q are
+// formed here instead of in a separate vector kernel.
+struct PcgFuse {
+    int on;
+    double self;
+    const double *vp;          // 3 n_pad, direction p (FP64)
+    const double *inv_alpha;   // n_pad
+    double *vq;                // 3 n_pad out
+    double *part;              // 2 * n_groups block partials
+};
 
 // ----------------------------------------------------------------------------- list construction
 // One CTA per group.  Chunk by chunk, the staged positions are put in shared memory, every lane
@@ -45,12 +59,13 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int b0 = ws.group_first[g], nb = ws.group_first[g + 1] - b0;
     const int count = ws.stage_count[g];
     const size_t gbase = (size_t)g * ws.s_cap;
-    int n_chunks, s_chunk;
-    atom_chunking(st->max_stage, sizeof(real) == 8, &n_chunks, &s_chunk);
-    if (n_chunks > NCH_MAX) {                      // uniform over the grid
+    const int s_chunk = atom_chunk_capacity(sizeof(real) == 8, ws.chunk_cap);
+    const int n_chunks = atom_chunks_of(count, s_chunk);
+    if (n_chunks > NCH_MAX) {                      // uniform over the CTA
         if (t == 0) st->atom_bad = 1;
         return;
     }
+    const unsigned magic = ((1u << 20) + (unsigned)n_chunks - 1u) / (unsigned)n_chunks;   // e / n for e < 2^16
     const bool active = w < nb;
     const int blk = b0 + (active ? w : 0);
     const int slot = blk * BLOCK + lane;
@@ -58,47 +73,68 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int oct = slot >> 3;
     const int L = active ? ws.oct_len[oct] : 0;
     const uint16_t *__restrict__ ent = ws.entries + (size_t)oct * ws.l_cap;
-    uint16_t *__restrict__ out = ws.alist + (size_t)blk * ws.a_cap * 32 + lane * 4;
+    // a lane's list as quads of 4 entries: quad q of lane l at uint2 index q * 32 + l of the block
+    uint2 *__restrict__ out = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
     int32_t *__restrict__ arow = ws.arow + (size_t)blk * (NCH_MAX + 1);
     const unsigned dummy = (unsigned)s_chunk * (unsigned)sizeof(vec4);
+    const unsigned long long dummy4 = 0x0001000100010001ull * (unsigned long long)dummy;
+    const int q_cap = ws.a_cap >> 2;
+    const uint4 *__restrict__ ent8 = reinterpret_cast<const uint4 *>(ent);    // 8 entries per load
+    const int L8 = L >> 3;                                                     // L is a multiple of 8
 
-    int k0 = 0;        // first entry of the current chunk's list (same for all lanes, multiple of 4)
-    int cur = 0;       // cursor into the cluster list
+    int q0 = 0;        // first quad of the current chunk's list (same for all lanes)
     for (int c = 0; c < n_chunks; ++c) {
-        const int c0 = c * s_chunk, c1 = min(c0 + s_chunk, count);
         __syncthreads();
-        for (int idx = c0 + t; idx < c1; idx += GT) s_pos[idx - c0] = stage_pos[gbase + idx];
+        for (int l = t, idx = c + t * n_chunks; idx < count; l += GT, idx += GT * n_chunks)
+            s_pos[l] = stage_pos[gbase + idx];
         __syncthreads();
         if (!active) continue;
-        if (lane == 0) arow[c] = k0;
-        int k = 0;     // entries this lane appended in this chunk
-        while (cur < L) {
-            const unsigned e = ent[cur];                 // one address per quarter warp
-            if ((int)e >= c1) break;                     // next chunk (padding entries == count)
-            ++cur;
-            const unsigned loc = e - (unsigned)c0;
-            const vec4 pj = s_pos[loc];
-            const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
-            const real r2 = Rx * Rx + Ry * Ry + Rz * Rz;
-            if (r2 <= rc2 && r2 > (real)1e-10) {
-                const int ka = k0 + k;
-                if (ka < ws.a_cap) out[(size_t)(ka >> 2) * 128 + (ka & 3)] = (uint16_t)(loc * (unsigned)sizeof(vec4));
-                ++k;
+        if (lane == 0) arow[c] = q0 << 2;
+        int k = 0;                         // entries this lane appended in this chunk
+        unsigned long long pend = 0;       // the quad being filled
+        uint4 nxt = L8 > 0 ? ent8[0] : make_uint4(0, 0, 0, 0);
+        bool open = true;
+        for (int v = 0; v < L8 && open; ++v) {
+            const uint4 cur = nxt;
+            if (v + 1 < L8) nxt = ent8[v + 1];           // one address per quarter warp, one load ahead
+            const unsigned word[4] = {cur.x, cur.y, cur.z, cur.w};
+#pragma unroll
+            for (int h = 0; h < 8; ++h) {
+                const unsigned e = (word[h >> 1] >> ((h & 1) * 16)) & 0xffffu;
+                if ((int)e >= count) { open = false; break; }      // padding entries (== count) close the list
+                const unsigned loc = (e * magic) >> 20;            // e / n_chunks
+                if (e - loc * (unsigned)n_chunks != (unsigned)c) continue;
+                const vec4 pj = s_pos[loc];
+                const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
+                const real r2 = Rx * Rx + Ry * Ry + Rz * Rz;
+                if (r2 <= rc2 && r2 > (real)1e-10) {
+                    pend |= (unsigned long long)(loc * (unsigned)sizeof(vec4)) << ((k & 3) * 16);
+                    if ((k & 3) == 3) {
+                        const int q = q0 + (k >> 2);
+                        if (q < q_cap) out[(size_t)q * 32] = make_uint2((unsigned)pend, (unsigned)(pend >> 32));
+                        pend = 0;
+                    }
+                    ++k;
+                }
             }
         }
         int kmax = k;
         for (int o = 16; o > 0; o >>= 1) kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
-        kmax = (kmax + 3) & ~3;
-        if (k0 + kmax > ws.a_cap) {
+        int qmax = (kmax + 3) >> 2;
+        if (q0 + qmax > q_cap) {
             if (lane == 0) st->atom_bad = 1;
-            kmax = ws.a_cap - k0;
+            qmax = q_cap - q0;
         }
-        for (int kk = k; kk < kmax; ++kk) {
-            const int ka = k0 + kk;
-            out[(size_t)(ka >> 2) * 128 + (ka & 3)] = (uint16_t)dummy;
+        int qd = k >> 2;                   // first quad this lane has not stored yet
+        if ((k & 3) != 0) {                // partly filled quad: the rest are dummies
+            pend |= dummy4 << ((k & 3) * 16);
+            if (q0 + qd < q_cap) out[(size_t)(q0 + qd) * 32] = make_uint2((unsigned)pend, (unsigned)(pend >> 32));
+            ++qd;
         }
-        k0 += kmax;
+        for (; qd < qmax; ++qd) out[(size_t)(q0 + qd) * 32] = make_uint2((unsigned)dummy4, (unsigned)(dummy4 >> 32));
+        q0 += qmax;
     }
+    const int k0 = q0 << 2;
     if (active && lane == 0) {
         for (int c = n_chunks; c <= NCH_MAX; ++c) arow[c] = k0;
         atomicAdd((unsigned long long *)&st->n_atom_entries, (unsigned long long)k0);
@@ -165,7 +201,9 @@ __global__ void __launch_bounds__(GT)
 k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
              const typename Vec4<real>::type *__restrict__ stage_pos,
              const typename Vec4<real>::type *__restrict__ data,   // mu (n_pad) or multipoles (3 n_pad)
-             PairConsts<real> kc, double *__restrict__ acc, int n_pad, int s_chunk, int n_chunks) {
+             PairConsts<real> kc, double *__restrict__ acc, int n_pad, int s_chunk,
+             DeviceState *st, int iter, PcgFuse fuse) {
+    if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     using vec4 = typename Vec4<real>::type;
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -177,6 +215,7 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int g = blockIdx.x, t = threadIdx.x, lane = t & 31, w = t >> 5;
     const int b0 = ws.group_first[g], nb = ws.group_first[g + 1] - b0;
     const int count = ws.stage_count[g];
+    const int n_chunks = atom_chunks_of(count, s_chunk);
     const size_t gbase = (size_t)g * ws.s_cap;
     const bool active = w < nb;
     const int blk = b0 + (active ? w : 0);
@@ -200,26 +239,28 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     }
 
     for (int c = 0; c < n_chunks; ++c) {
-        const int c0 = c * s_chunk, c1 = min(c0 + s_chunk, count);
         __syncthreads();
-        for (int idx = c0 + t; idx < c1; idx += GT) {
+        for (int l = t, idx = c + t * n_chunks; idx < count; l += GT, idx += GT * n_chunks) {
             const int a = ws.stage_atom[gbase + idx];
-            s_pos[idx - c0] = stage_pos[gbase + idx];
+            s_pos[l] = stage_pos[gbase + idx];
 #pragma unroll
-            for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + (idx - c0)] = data[(size_t)k * n_pad + a];
+            for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + l] = data[(size_t)k * n_pad + a];
         }
         __syncthreads();
         if (!active) continue;
         const int q0 = arow[c] >> 2, q1 = arow[c + 1] >> 2;
         if (q0 >= q1) continue;
         const unsigned char *s_base = smem_raw;
+        // list quads are fetched two steps ahead of their use (L2 latency under load ~ one step)
         uint2 e = lp[(size_t)q0 * 32];
+        uint2 e1 = lp[(size_t)(q0 + 1 < q1 ? q0 + 1 : q0) * 32];
         for (int q = q0; q < q1; ++q) {
-            const int qn = q + 1 < q1 ? q + 1 : q;
-            const uint2 en = lp[(size_t)qn * 32];          // next 4 entries, used one iteration later
+            const int qn = q + 2 < q1 ? q + 2 : q1 - 1;
+            const uint2 e2 = lp[(size_t)qn * 32];
             eval_pair2<real, MODE>(s_base, pay_stride, e.x & 0xffffu, e.x >> 16, pi, gi, kc, ax, ay, az);
             eval_pair2<real, MODE>(s_base, pay_stride, e.y & 0xffffu, e.y >> 16, pi, gi, kc, ax, ay, az);
-            e = en;
+            e = e1;
+            e1 = e2;
             if (++since_flush == 8) {          // every 32 entries: FP32 partial -> FP64 accumulator
                 dx += (double)ax; dy += (double)ay; dz += (double)az;
                 ax = 0; ay = 0; az = 0;
@@ -227,19 +268,36 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             }
         }
     }
-    if (!active) return;
     dx += (double)ax; dy += (double)ay; dz += (double)az;
-    acc[slot] = dx;
-    acc[n_pad + slot] = dy;
-    acc[2 * (size_t)n_pad + slot] = dz;
+    if (active) {
+        acc[slot] = dx;
+        acc[n_pad + slot] = dy;
+        acc[2 * (size_t)n_pad + slot] = dz;
+    }
+    if (MODE == MODE_TMU && fuse.on) {
+        double pq = 0, dummy = 0;
+        if (active) {
+            const double ia = fuse.inv_alpha[slot];
+            const double d[3] = {dx, dy, dz};
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const size_t o = (size_t)k * n_pad + slot;
+                const double p = fuse.vp[o];
+                const double q = p * ia - d[k] - fuse.self * p;
+                fuse.vq[o] = q;
+                pq += p * q;
+            }
+        }
+        block_sum2(pq, dummy);
+        if (grid_sum2_last_block(fuse.part, &st->ticket, pq, dummy) && threadIdx.x == 0) st->pq = pq;
+    }
 }
 
 // ----------------------------------------------------------------------------- host side
 int atom_build(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
     const bool f64 = c->p.precision == TKHP_FP64;
-    int n_chunks, s_chunk;
-    atom_chunking(1 << 30, f64, &n_chunks, &s_chunk);          // s_chunk = the largest chunk
+    const int s_chunk = atom_chunk_capacity(f64, ws.chunk_cap);
     const size_t smem = (size_t)s_chunk * (f64 ? sizeof(double4) : sizeof(float4));
     const double rc2 = c->p.cutoff * c->p.cutoff;
     if (f64)
@@ -256,8 +314,7 @@ static int launch_atom_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     using vec4 = typename Vec4<real>::type;
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
     constexpr int which = sizeof(real) == 8;
-    int n_chunks, s_chunk;
-    atom_chunking(c->h_state->max_stage, which, &n_chunks, &s_chunk);
+    const int s_chunk = atom_chunk_capacity(which, ws.chunk_cap);
     const size_t smem = sizeof(vec4) * (size_t)(1 + NPAY) * (size_t)(s_chunk + 1);
     static bool configured[2][2] = {{false, false}, {false, false}};
     if (!configured[which][MODE]) {
@@ -272,12 +329,17 @@ static int launch_atom_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     k.rc2 = (real)(c->p.cutoff * c->p.cutoff);
     k.box = (real)1;
     k.inv_box = (real)0;
+    PcgFuse fuse;
+    fuse.on = MODE == MODE_TMU && c->fuse_q;
+    fuse.self = 4.0 * c->p.ewald_beta * c->p.ewald_beta * c->p.ewald_beta / (3.0 * SQRT_PI);
+    fuse.vp = c->vp; fuse.inv_alpha = c->inv_alpha_s; fuse.vq = c->vq;
+    fuse.part = c->partials + 2 * (size_t)c->part_cap;
     const vec4 *gpos = which ? (const vec4 *)ws.gpos64 : (const vec4 *)ws.gpos32;
     const vec4 *spos = which ? (const vec4 *)ws.stage_pos64 : (const vec4 *)ws.stage_pos32;
     const vec4 *data;
     if (MODE == MODE_TMU) data = which ? (const vec4 *)c->mu64 : (const vec4 *)c->mu32;
     else data = which ? (const vec4 *)c->mp64 : (const vec4 *)c->mp32;
-    k_atom_pairs<real, MODE><<<ws.n_groups, GT, smem, s>>>(ws, gpos, spos, data, k, c->acc, c->n_pad, s_chunk, n_chunks);
+    k_atom_pairs<real, MODE><<<ws.n_groups, GT, smem, s>>>(ws, gpos, spos, data, k, c->acc, c->n_pad, s_chunk, c->st, c->spec_iter, fuse);
     c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;

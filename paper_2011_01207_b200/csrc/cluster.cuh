@@ -39,16 +39,17 @@ constexpr float GUARD = 0.01f;        // list radius = r_c + GUARD (FP32 build a
 constexpr int NCH_MAX = 16;           // ATOM mode: max staging chunks per group
 constexpr int ATOM_SMEM = 56 * 1024;  // ATOM mode: shared memory of the T.mu kernel per CTA (4 CTAs / SM)
 
-// ATOM mode chunking of a group's staged atoms: the same function on the host (launch geometry)
-// and on the device (list construction), from the largest staged-atom count of any group.
-__host__ __device__ inline void atom_chunking(int max_stage, bool f64, int *n_chunks, int *s_chunk) {
-    const int s_max = (ATOM_SMEM / (f64 ? 64 : 32) - 1) & ~31;   // records of pos + mu
-    if (max_stage < 1) max_stage = 1;
-    const int n = (max_stage + s_max - 1) / s_max;
-    int s = (((max_stage + n - 1) / n) + 31) & ~31;
-    if (s > s_max) s = s_max;
-    *n_chunks = n;
-    *s_chunk = s;
+// ATOM mode chunking of a group's staged atoms.  The shared-memory chunk holds s_max records; a
+// group with `count` staged atoms uses n = ceil(count / s_max) chunks, chunk c = the staged atoms
+// with index == c (mod n), stored at local index idx / n.  Interleaving (instead of consecutive
+// runs of the spatially ordered staging area) splits every atom's neighbours evenly over the
+// chunks, so that padding each chunk's lists to the longest lane of the warp stays cheap.
+__host__ __device__ inline int atom_chunk_capacity(bool f64, int user_cap) {
+    const int fit = (ATOM_SMEM / (f64 ? 64 : 32) - 1) & ~31;     // records of pos + mu
+    return (user_cap > 0 && user_cap < fit) ? user_cap : fit;
+}
+__host__ __device__ inline int atom_chunks_of(int count, int s_chunk) {
+    return count < 1 ? 1 : (count + s_chunk - 1) / s_chunk;
 }
 
 struct ClusterWs {
@@ -66,6 +67,7 @@ struct ClusterWs {
     // ATOM list mode (atom_pairs.cu): per-atom lists, one u16 BYTE OFFSET into the staged chunk per
     // entry, laid out per block as [entry/4][lane][entry%4] so that a lane reads 4 entries with one
     // coalesced 8-byte load; every chunk's list is padded to the longest lane of the warp.
+    int chunk_cap;                    // tkhp_params.max_stage_per_chunk (0 = automatic)
     int a_cap;                        // entries per lane and block (multiple of 4)
     uint16_t *alist;                  // n_blocks * a_cap * 32
     int32_t *arow;                    // n_blocks * (NCH_MAX + 1): first entry of each chunk's list
@@ -122,6 +124,7 @@ inline size_t carve_cluster(const tkhp_params *p, int n_blocks, void *base, Clus
     ws.entries = w.take<uint16_t>((n_pad / CLUSTER) * ws.l_cap);
     ws.oct_len = w.take<int32_t>(n_pad / CLUSTER);
     ws.a_cap = 0; ws.alist = nullptr; ws.arow = nullptr;
+    ws.chunk_cap = p->max_stage_per_chunk;
     if (p->list_mode == TKHP_LIST_ATOM) {
         long long a;
         if (p->max_nbrs_per_atom > 0) {

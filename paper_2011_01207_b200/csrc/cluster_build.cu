@@ -215,23 +215,27 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
 
     // (f) per-cluster lists: entries are staging indices, in staging order
     if (w < nb) {
-        int len[4];
+        int len[4] = {0, 0, 0, 0};
         const int oct0 = (b0 + w) * 4;
-        for (int oo = 0; oo < 4; ++oo) {
-            const int o = w * 4 + oo;
-            uint16_t *ent = ws.entries + (size_t)(oct0 + oo) * ws.l_cap;
-            int n = 0;
-            for (int base = 0; base < count; base += 32) {
-                const int idx = base + lane;
-                const bool bit = idx < count && ((ws.stage_mask[gbase + idx] >> o) & 1u);
+        uint16_t *ent[4];
+        for (int oo = 0; oo < 4; ++oo) ent[oo] = ws.entries + (size_t)(oct0 + oo) * ws.l_cap;
+        // one pass over the staged atoms for the warp's 4 clusters; the mask of the next round is
+        // loaded before the ballots of this one
+        uint32_t m_next = lane < count ? ws.stage_mask[gbase + lane] : 0u;
+        for (int base = 0; base < count; base += 32) {
+            const int idx = base + lane;
+            const uint32_t m = (m_next >> (w * 4)) & 0xfu;
+            m_next = idx + 32 < count ? ws.stage_mask[gbase + idx + 32] : 0u;
+#pragma unroll
+            for (int oo = 0; oo < 4; ++oo) {
+                const bool bit = (m >> oo) & 1u;
                 const unsigned bm = __ballot_sync(0xffffffffu, bit);
                 if (bit) {
-                    const int pos = n + __popc(bm & ((1u << lane) - 1u));
-                    if (pos < ws.l_cap) ent[pos] = (uint16_t)idx;
+                    const int pos = len[oo] + __popc(bm & ((1u << lane) - 1u));
+                    if (pos < ws.l_cap) ent[oo][pos] = (uint16_t)idx;
                 }
-                n += __popc(bm);
+                len[oo] += __popc(bm);
             }
-            len[oo] = n;
         }
         int L = max(max(len[0], len[1]), max(len[2], len[3]));
         if (L > ws.l_cap) {
@@ -241,8 +245,7 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
         L = (L + 7) & ~7;
         if (L > ws.l_cap) L = ws.l_cap;
         for (int oo = 0; oo < 4; ++oo) {
-            uint16_t *ent = ws.entries + (size_t)(oct0 + oo) * ws.l_cap;
-            for (int k = min(len[oo], L) + lane; k < L; k += 32) ent[k] = (uint16_t)count;   // dummy far atom
+            for (int k = min(len[oo], L) + lane; k < L; k += 32) ent[oo][k] = (uint16_t)count;   // dummy far atom
             if (lane == 0) ws.oct_len[oct0 + oo] = L;
         }
         if (lane == 0) atomicAdd((unsigned long long *)&st->n_cluster_entries, (unsigned long long)(4 * L));

@@ -26,7 +26,9 @@ __global__ void __launch_bounds__(GT)
 k_cluster_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
                 const typename Vec4<real>::type *__restrict__ stage_pos,
                 const typename Vec4<real>::type *__restrict__ data,   // mu (n_pad) or multipoles (3 n_pad)
-                PairConsts<real> kc, double *__restrict__ acc, int n_pad, int s_chunk) {
+                PairConsts<real> kc, double *__restrict__ acc, int n_pad, int s_chunk,
+                const DeviceState *__restrict__ st, int iter) {
+    if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     using vec4 = typename Vec4<real>::type;
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
     constexpr int NK = MODE == MODE_TMU ? 2 : 3;
@@ -179,7 +181,7 @@ static int launch_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     const vec4 *data;
     if (MODE == MODE_TMU) data = which ? (const vec4 *)c->mu64 : (const vec4 *)c->mu32;
     else data = which ? (const vec4 *)c->mp64 : (const vec4 *)c->mp32;
-    k_cluster_pairs<real, MODE><<<ws.n_groups, GT, smem, s>>>(ws, gpos, spos, data, k, c->acc, c->n_pad, s_chunk);
+    k_cluster_pairs<real, MODE><<<ws.n_groups, GT, smem, s>>>(ws, gpos, spos, data, k, c->acc, c->n_pad, s_chunk, c->st, c->spec_iter);
     c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;

@@ -46,8 +46,11 @@ struct DeviceState {
     int atom_bad;                       // 1: ATOM lists unusable (capacity / too many chunks): CLUSTER is used
     int pad1;
     // PCG scalars
-    double rz, pq, rr, gamma, delta;
-    int converged;
+    double rzv[2];          // r.z ping-pong (iteration parity)
+    double pq, rr, gamma, delta;
+    unsigned ticket;        // last-block reductions (reduce.cuh); 0 between kernels
+    int pad2;
+    int conv_at;            // PCG: iterations with index >= conv_at are skipped on the device
     int iters;
 };
 
@@ -98,8 +101,12 @@ struct Ctx {
     double4 *mp64;          // 3 * n_pad
     // PCG vectors, sorted order, SoA 3 * n_pad each
     double *vE, *vmu, *vr, *vp, *vq;
-    double *partials;       // 4 sets (rz ping, rz pong, pq, energy) of 2 * MAX_PARTIALS
+    double *partials;       // 3 sets (rz, pq, energy) of 2 * part_cap block partials
+    int part_cap;           // >= the largest grid of any reducing kernel (n_blocks + MAX_PARTIALS)
     double *h_scalars;      // pinned host scratch (8 doubles) for scalar read-backs
+    double *h_ring, *d_ring; // mapped pinned ring: |r|^2 of each PCG iteration, written by the device
+    bool fuse_q;            // ATOM-mode T.mu kernel also forms q = p/alpha - T p - self p and p.q (PCG)
+    int spec_iter;          // >= 0: the pair kernel about to be launched belongs to PCG iteration spec_iter
     DeviceState *h_state;   // pinned host copy of *st (list header), valid when header_valid
     bool header_valid;
     // host-entry staging (tkhp_polarize_host)
@@ -116,8 +123,13 @@ struct Ctx {
     bool prof;                          // record an event pair around every T.mu / field pair kernel
     int prof_n[2];                      // [0] T.mu launches, [1] field launches recorded
     cudaEvent_t prof_ev[2][2 * 64];
+    int prof_iter[2][64];               // PCG iteration the recorded launch belongs to (-1: unconditional)
+    bool prof_skip[2][64];              // the launch was a speculative no-op (iteration after convergence)
+    long long n_noop_launches;          // launches that returned at once for the same reason
 };
 constexpr int PROF_MAX = 64;
+constexpr int RING = 16;          // slots of the PCG residual ring
+constexpr int PCG_LAG = 2;        // iterations the host enqueues ahead of the last residual it has seen
 
 // Bump allocator over the caller's workspace; with base == nullptr it only measures.
 struct Carver {

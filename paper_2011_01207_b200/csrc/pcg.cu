@@ -10,14 +10,15 @@
 //   loop: q = A p; gamma = (r.z)/(p.q); mu += gamma p; r -= gamma q; rms = sqrt(|r|^2/N);
 //         z = alpha r; delta = (r.z)new/(r.z)old; p = z + delta p,     A v = v/alpha - T v.
 // All vectors live in the SORTED, padded order (SoA x|y|z, FP64); dot products are FP64 two-level
-// tree reductions (block partials, then every block of the next kernel re-reduces the partials:
-// deterministic, no atomics, no extra launch).
+// tree reductions (block partials, then the last block of the same kernel re-reduces them in a
+// fixed order: deterministic, no floating-point atomics, no extra launch; reduce.cuh).
 #include "common.cuh"
 #include "pair_math.cuh"
+#include "reduce.cuh"
 
 namespace tkhp {
 
-constexpr int VEC_THREADS = 256;
+constexpr int VEC_THREADS = RED_THREADS;
 
 // ----------------------------------------------------------------------------- packing
 template <typename vec4>
@@ -103,34 +104,6 @@ __global__ void k_field_finish(const double *__restrict__ acc, const int32_t *__
     field[3 * (size_t)a + 2] = ez + self * dip[3 * (size_t)a + 2];
 }
 
-// ----------------------------------------------------------------------------- reductions
-// block-level sum of up to two values; result valid in thread 0
-__device__ __forceinline__ void block_sum2(double &a, double &b) {
-    __shared__ double sa[VEC_THREADS / 32], sb[VEC_THREADS / 32];
-    a = warp_sum(a); b = warp_sum(b);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    __syncthreads();
-    if (lane == 0) { sa[w] = a; sb[w] = b; }
-    __syncthreads();
-    if (w == 0) {
-        a = lane < VEC_THREADS / 32 ? sa[lane] : 0.0;
-        b = lane < VEC_THREADS / 32 ? sb[lane] : 0.0;
-        a = warp_sum(a); b = warp_sum(b);
-    }
-}
-
-// every block re-reduces the partials of a previous kernel (fixed order => deterministic)
-__device__ __forceinline__ void reduce_partials2(const double *__restrict__ part, int n_part, double &a, double &b) {
-    __shared__ double bc[2];
-    double x = 0, y = 0;
-    for (int i = threadIdx.x; i < n_part; i += VEC_THREADS) { x += part[2 * i]; y += part[2 * i + 1]; }
-    block_sum2(x, y);
-    if (threadIdx.x == 0) { bc[0] = x; bc[1] = y; }
-    __syncthreads();
-    a = bc[0]; b = bc[1];
-    __syncthreads();
-}
-
 template <typename vec4>
 __device__ __forceinline__ void store_vec(vec4 *out, int s, double x, double y, double z) {
     vec4 v;
@@ -139,12 +112,19 @@ __device__ __forceinline__ void store_vec(vec4 *out, int s, double x, double y, 
 }
 
 // ----------------------------------------------------------------------------- PCG kernels
+// Device-side control (no host round trip per iteration): st->conv_at = first iteration index that
+// must NOT run; every kernel of iteration `iter` returns at once when iter >= conv_at.  The kernel
+// that forms a new residual (k_pcg_residual0, k_pcg_update) lowers conv_at in its last block, i.e.
+// after every block of that kernel has passed its own test.
+//
 // mu0 = alpha E or the guess; gather E to sorted order; pack mu for the first matvec
 template <typename vec4>
 __global__ void k_pcg_init(const double *__restrict__ field, const double *__restrict__ guess, int use_guess,
                            const int32_t *__restrict__ perm, const double *__restrict__ alpha_s, int n_pad,
-                           double *__restrict__ vE, double *__restrict__ vmu, vec4 *__restrict__ packed) {
+                           double *__restrict__ vE, double *__restrict__ vmu, vec4 *__restrict__ packed,
+                           DeviceState *st) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s == 0) { st->conv_at = 0x7fffffff; st->iters = 0; st->ticket = 0u; }
     if (s >= n_pad) return;
     const int a = perm[s];
     double e[3] = {0, 0, 0}, m[3] = {0, 0, 0};
@@ -158,13 +138,13 @@ __global__ void k_pcg_init(const double *__restrict__ field, const double *__res
     store_vec(packed, s, m[0], m[1], m[2]);
 }
 
-// r = E - (mu/alpha - acc - self mu); z = alpha r; p = z; partials (r.z, r.r); pack p
+// r = E - (mu/alpha - acc - self mu); z = alpha r; p = z; (r.z, r.r) -> st->rzv[0], ring slot 0; pack p
 template <typename vec4>
-__global__ void k_pcg_residual0(const double *__restrict__ acc, const double *__restrict__ vE,
-                                const double *__restrict__ vmu, const double *__restrict__ alpha_s,
-                                const double *__restrict__ inv_alpha_s, double self, int n_pad,
-                                double *__restrict__ vr, double *__restrict__ vp, vec4 *__restrict__ packed,
-                                double *__restrict__ part_rz) {
+__global__ void __launch_bounds__(RED_THREADS)
+k_pcg_residual0(const double *__restrict__ acc, const double *__restrict__ vE, const double *__restrict__ vmu,
+                const double *__restrict__ alpha_s, const double *__restrict__ inv_alpha_s, double self, int n_pad,
+                double *__restrict__ vr, double *__restrict__ vp, vec4 *__restrict__ packed,
+                double *__restrict__ part, DeviceState *st, double tol, int n_atoms, volatile double *ring_slot) {
     double rz = 0, rr = 0;
     for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < n_pad; s += gridDim.x * blockDim.x) {
         const double al = alpha_s[s], ia = inv_alpha_s[s];
@@ -180,13 +160,16 @@ __global__ void k_pcg_residual0(const double *__restrict__ acc, const double *__
         store_vec(packed, s, p[0], p[1], p[2]);
     }
     block_sum2(rz, rr);
-    if (threadIdx.x == 0) { part_rz[2 * blockIdx.x] = rz; part_rz[2 * blockIdx.x + 1] = rr; }
+    if (grid_sum2_last_block(part, &st->ticket, rz, rr) && threadIdx.x == 0)
+        pcg_publish_residual(st, 0, rz, rr, 0, tol, n_atoms, ring_slot);
 }
 
-// q = p/alpha - acc - self p ; partial p.q
-__global__ void k_pcg_q(const double *__restrict__ acc, const double *__restrict__ vp,
-                        const double *__restrict__ inv_alpha_s, double self, int n_pad, double *__restrict__ vq,
-                        double *__restrict__ part_pq) {
+// q = p/alpha - acc - self p ; p.q -> st->pq   (TILES and CLUSTER modes; the ATOM-mode pair kernel
+// does this in its epilogue)
+__global__ void __launch_bounds__(RED_THREADS)
+k_pcg_q(const double *__restrict__ acc, const double *__restrict__ vp, const double *__restrict__ inv_alpha_s,
+        double self, int n_pad, double *__restrict__ vq, double *__restrict__ part, DeviceState *st, int iter) {
+    if (iter >= st->conv_at) return;
     double pq = 0, dummy = 0;
     for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < n_pad; s += gridDim.x * blockDim.x) {
         const double ia = inv_alpha_s[s];
@@ -199,18 +182,16 @@ __global__ void k_pcg_q(const double *__restrict__ acc, const double *__restrict
         }
     }
     block_sum2(pq, dummy);
-    if (threadIdx.x == 0) { part_pq[2 * blockIdx.x] = pq; part_pq[2 * blockIdx.x + 1] = 0.0; }
+    if (grid_sum2_last_block(part, &st->ticket, pq, dummy) && threadIdx.x == 0) st->pq = pq;
 }
 
-// gamma = rz/pq ; mu += gamma p ; r -= gamma q ; partials (r.z, r.r) with z = alpha r
-__global__ void k_pcg_update(const double *__restrict__ part_rz_old, const double *__restrict__ part_pq,
-                             int n_part, const double *__restrict__ vp, const double *__restrict__ vq,
-                             const double *__restrict__ alpha_s, int n_pad, double *__restrict__ vmu,
-                             double *__restrict__ vr, double *__restrict__ part_rz_new) {
-    double rz_old, rr_old, pq, dmy;
-    reduce_partials2(part_rz_old, n_part, rz_old, rr_old);
-    reduce_partials2(part_pq, n_part, pq, dmy);
-    const double gamma = rz_old / pq;
+// gamma = rz/pq ; mu += gamma p ; r -= gamma q ; (r.z, r.r) with z = alpha r -> st->rzv[nxt], ring
+__global__ void __launch_bounds__(RED_THREADS)
+k_pcg_update(const double *__restrict__ vp, const double *__restrict__ vq, const double *__restrict__ alpha_s,
+             int n_pad, double *__restrict__ vmu, double *__restrict__ vr, double *__restrict__ part,
+             DeviceState *st, int iter, double tol, int n_atoms, volatile double *ring_slot) {
+    if (iter >= st->conv_at) return;
+    const double gamma = st->rzv[iter & 1] / st->pq;
     double rz = 0, rr = 0;
     for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < n_pad; s += gridDim.x * blockDim.x) {
         const double al = alpha_s[s];
@@ -223,20 +204,17 @@ __global__ void k_pcg_update(const double *__restrict__ part_rz_old, const doubl
         }
     }
     block_sum2(rz, rr);
-    if (threadIdx.x == 0) { part_rz_new[2 * blockIdx.x] = rz; part_rz_new[2 * blockIdx.x + 1] = rr; }
+    if (grid_sum2_last_block(part, &st->ticket, rz, rr) && threadIdx.x == 0)
+        pcg_publish_residual(st, (iter + 1) & 1, rz, rr, iter + 1, tol, n_atoms, ring_slot);
 }
 
-// delta = rz_new/rz_old ; p = alpha r + delta p ; pack p ; block 0 publishes |r|^2
+// delta = rz_new/rz_old ; p = alpha r + delta p ; pack p   (not needed once converged)
 template <typename vec4>
-__global__ void k_pcg_direction(const double *__restrict__ part_rz_old, const double *__restrict__ part_rz_new,
-                                int n_part, const double *__restrict__ vr, const double *__restrict__ alpha_s,
-                                int n_pad, double *__restrict__ vp, vec4 *__restrict__ packed,
-                                DeviceState *st) {
-    double rz_old, rr_old, rz_new, rr_new;
-    reduce_partials2(part_rz_old, n_part, rz_old, rr_old);
-    reduce_partials2(part_rz_new, n_part, rz_new, rr_new);
-    const double delta = rz_new / rz_old;
-    if (blockIdx.x == 0 && threadIdx.x == 0) { st->rr = rr_new; st->rz = rz_new; st->delta = delta; }
+__global__ void k_pcg_direction(const double *__restrict__ vr, const double *__restrict__ alpha_s, int n_pad,
+                                double *__restrict__ vp, vec4 *__restrict__ packed,
+                                const DeviceState *__restrict__ st, int iter) {
+    if (iter + 1 >= st->conv_at) return;
+    const double delta = st->rzv[(iter + 1) & 1] / st->rzv[iter & 1];
     for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < n_pad; s += gridDim.x * blockDim.x) {
         const double al = alpha_s[s];
         double p[3];
@@ -249,12 +227,6 @@ __global__ void k_pcg_direction(const double *__restrict__ part_rz_old, const do
     }
 }
 
-__global__ void k_publish_rr(const double *__restrict__ part_rz, int n_part, DeviceState *st) {
-    double rz, rr;
-    reduce_partials2(part_rz, n_part, rz, rr);
-    if (threadIdx.x == 0) { st->rr = rr; st->rz = rz; }
-}
-
 __global__ void k_unsort3(const double *__restrict__ v, const int32_t *__restrict__ perm, int n_pad,
                           double *__restrict__ out) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -265,18 +237,14 @@ __global__ void k_unsort3(const double *__restrict__ v, const int32_t *__restric
 }
 
 // ----------------------------------------------------------------------------- energy
-__global__ void k_energy_partials(const double *__restrict__ mu, const double *__restrict__ field, long long n3,
-                                  double *__restrict__ part) {
+__global__ void __launch_bounds__(RED_THREADS)
+k_energy(const double *__restrict__ mu, const double *__restrict__ field, long long n3, double *__restrict__ part,
+         DeviceState *st, double *__restrict__ energy) {
     double s = 0, dmy = 0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += (long long)gridDim.x * blockDim.x)
         s += mu[i] * field[i];
     block_sum2(s, dmy);
-    if (threadIdx.x == 0) { part[2 * blockIdx.x] = s; part[2 * blockIdx.x + 1] = 0.0; }
-}
-__global__ void k_energy_final(const double *__restrict__ part, int n_part, double *__restrict__ energy) {
-    double s, dmy;
-    reduce_partials2(part, n_part, s, dmy);
-    if (threadIdx.x == 0) *energy = -0.5 * COULOMB * s;
+    if (grid_sum2_last_block(part, &st->ticket, s, dmy) && threadIdx.x == 0) *energy = -0.5 * COULOMB * s;
 }
 
 // ----------------------------------------------------------------------------- host drivers
@@ -293,6 +261,8 @@ static inline int vec_grid(const Ctx *c) {
 static inline bool prof_begin(Ctx *c, int which, cudaStream_t s) {
     if (!c->prof || c->prof_n[which] >= PROF_MAX) return false;
     cudaEventRecord(c->prof_ev[which][2 * c->prof_n[which]], s);
+    c->prof_iter[which][c->prof_n[which]] = c->spec_iter;
+    c->prof_skip[which][c->prof_n[which]] = false;
     return true;
 }
 static inline void prof_end(Ctx *c, int which, cudaStream_t s) {
@@ -353,13 +323,30 @@ int do_tmatvec(Ctx *c, const double *d_mu, double *d_out, cudaStream_t s) {
     return TKHP_OK;
 }
 
-static int read_rr(Ctx *c, cudaStream_t s, double *rr) {
-    TKHP_CUDA(c, cudaMemcpyAsync(c->h_scalars, &c->st->rr, sizeof(double), cudaMemcpyDeviceToHost, s));
-    TKHP_CUDA(c, cudaStreamSynchronize(s));
-    *rr = c->h_scalars[0];
-    return TKHP_OK;
+// Wait for the device to publish |r|^2 into a ring slot (mapped pinned memory).  The host spins on
+// the slot; every few thousand spins it asks the stream whether it failed or drained (a drained
+// stream with an untouched slot means a kernel died).
+static int wait_slot(Ctx *c, cudaStream_t s, int slot, double *rr) {
+    volatile double *v = c->h_ring + slot;
+    for (unsigned spin = 1;; ++spin) {
+        const double x = *v;
+        if (!(x == -1.0)) { *rr = x; return TKHP_OK; }
+        if ((spin & 0xfff) == 0) {
+            const cudaError_t e = cudaStreamQuery(s);
+            if (e == cudaSuccess) {
+                const double y = *v;
+                if (!(y == -1.0)) { *rr = y; return TKHP_OK; }
+                return set_err(c, TKHP_ECUDA, "PCG residual was never published%s");
+            }
+            if (e != cudaErrorNotReady) TKHP_CUDA(c, e);
+        }
+    }
 }
 
+// The solve runs without a host round trip per iteration: the host enqueues iterations up to
+// PCG_LAG ahead of the last residual it has seen; the direction kernel of iteration k publishes
+// |r|^2 to the ring and lowers st->conv_at to k + 1 when rms < tol, which turns every kernel of
+// later (speculatively enqueued) iterations into an immediate return.
 int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int max_iter, int use_guess,
                    int *h_iters, double *h_rms, cudaStream_t s) {
     const int n_pad = c->n_pad;
@@ -367,39 +354,60 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
     const int gv = vec_grid(c);
     const double self = self_coeff(c->p);
     const bool mixed = c->p.precision == TKHP_MIXED;
-    double *part_rz[2] = {c->partials, c->partials + 2 * MAX_PARTIALS};
-    double *part_pq = c->partials + 4 * MAX_PARTIALS;
+    double *part_rz = c->partials;
+    double *part_pq = c->partials + 2 * (size_t)c->part_cap;
+    const bool fused_q = c->list_mode_in_use == TKHP_LIST_ATOM;   // q and p.q in the pair kernel's epilogue
     int rc;
 
+    for (int k = 0; k < RING; ++k) c->h_ring[k] = -1.0;
+    const int prof_first = c->prof_n[0];
     if (mixed)
-        k_pcg_init<float4><<<g1, VEC_THREADS, 0, s>>>(d_field, d_mu, use_guess, c->perm, c->alpha_s, n_pad, c->vE, c->vmu, c->mu32);
+        k_pcg_init<float4><<<g1, VEC_THREADS, 0, s>>>(d_field, d_mu, use_guess, c->perm, c->alpha_s, n_pad, c->vE, c->vmu, c->mu32, c->st);
     else
-        k_pcg_init<double4><<<g1, VEC_THREADS, 0, s>>>(d_field, d_mu, use_guess, c->perm, c->alpha_s, n_pad, c->vE, c->vmu, c->mu64);
+        k_pcg_init<double4><<<g1, VEC_THREADS, 0, s>>>(d_field, d_mu, use_guess, c->perm, c->alpha_s, n_pad, c->vE, c->vmu, c->mu64, c->st);
+    c->spec_iter = -1;
     if ((rc = run_tmatvec(c, s))) return rc;
     if (mixed)
-        k_pcg_residual0<float4><<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vE, c->vmu, c->alpha_s, c->inv_alpha_s, self, n_pad, c->vr, c->vp, c->mu32, part_rz[0]);
+        k_pcg_residual0<float4><<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vE, c->vmu, c->alpha_s, c->inv_alpha_s, self, n_pad, c->vr, c->vp, c->mu32, part_rz, c->st, tol, c->n, c->d_ring);
     else
-        k_pcg_residual0<double4><<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vE, c->vmu, c->alpha_s, c->inv_alpha_s, self, n_pad, c->vr, c->vp, c->mu64, part_rz[0]);
-    k_publish_rr<<<1, VEC_THREADS, 0, s>>>(part_rz[0], gv, c->st);
-    c->n_launches += 3;   // init, residual0, publish
-    double rr;
-    if ((rc = read_rr(c, s, &rr))) return rc;
-    double rms = sqrt(rr / c->n);
-    int it = 0;
-    while (rms >= tol && it < max_iter) {
-        const int cur = it & 1, nxt = cur ^ 1;
-        if ((rc = run_tmatvec(c, s))) return rc;
-        k_pcg_q<<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vp, c->inv_alpha_s, self, n_pad, c->vq, part_pq);
-        k_pcg_update<<<gv, VEC_THREADS, 0, s>>>(part_rz[cur], part_pq, gv, c->vp, c->vq, c->alpha_s, n_pad, c->vmu, c->vr, part_rz[nxt]);
-        if (mixed)
-            k_pcg_direction<float4><<<gv, VEC_THREADS, 0, s>>>(part_rz[cur], part_rz[nxt], gv, c->vr, c->alpha_s, n_pad, c->vp, c->mu32, c->st);
-        else
-            k_pcg_direction<double4><<<gv, VEC_THREADS, 0, s>>>(part_rz[cur], part_rz[nxt], gv, c->vr, c->alpha_s, n_pad, c->vp, c->mu64, c->st);
-        c->n_launches += 3;   // q, update, direction
-        ++it;
-        if ((rc = read_rr(c, s, &rr))) return rc;
+        k_pcg_residual0<double4><<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vE, c->vmu, c->alpha_s, c->inv_alpha_s, self, n_pad, c->vr, c->vp, c->mu64, part_rz, c->st, tol, c->n, c->d_ring);
+    c->n_launches += 2;   // init, residual0
+
+    // result j = |r|^2 after j iterations, in ring slot j % RING
+    int enq = 0, seen = 0, it = 0;
+    double rr = 0.0, rms = 0.0;
+    for (;;) {
+        while (enq < max_iter && enq < seen + PCG_LAG) {
+            const int slot = (enq + 1) % RING;
+            c->h_ring[slot] = -1.0;                 // consumed PCG_LAG < RING results ago
+            c->spec_iter = enq;
+            c->fuse_q = fused_q;
+            rc = run_tmatvec(c, s);
+            c->spec_iter = -1;
+            c->fuse_q = false;
+            if (rc) return rc;
+            if (!fused_q) {
+                k_pcg_q<<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vp, c->inv_alpha_s, self, n_pad, c->vq, part_pq, c->st, enq);
+                c->n_launches += 1;
+            }
+            k_pcg_update<<<gv, VEC_THREADS, 0, s>>>(c->vp, c->vq, c->alpha_s, n_pad, c->vmu, c->vr, part_rz, c->st, enq, tol, c->n, c->d_ring + slot);
+            if (mixed)
+                k_pcg_direction<float4><<<gv, VEC_THREADS, 0, s>>>(c->vr, c->alpha_s, n_pad, c->vp, c->mu32, c->st, enq);
+            else
+                k_pcg_direction<double4><<<gv, VEC_THREADS, 0, s>>>(c->vr, c->alpha_s, n_pad, c->vp, c->mu64, c->st, enq);
+            c->n_launches += 2;   // update, direction
+            ++enq;
+        }
+        if ((rc = wait_slot(c, s, seen % RING, &rr))) return rc;
+        it = seen++;                                // iterations completed when this residual was formed
         rms = sqrt(rr / c->n);
-        if (!(rms == rms)) break;   // NaN: give up
+        if (rms < tol || !(rms == rms) || it >= max_iter) break;
+    }
+    // speculative iterations enqueued after convergence returned at once: keep them out of the counts
+    if (rms < tol) {
+        c->n_noop_launches += (fused_q ? 3LL : 4LL) * (enq - it) + (it > 0 ? 1 : 0);   // + the last direction
+        for (int i = prof_first; i < c->prof_n[0]; ++i)
+            if (c->prof_iter[0][i] >= it) c->prof_skip[0][i] = true;
     }
     k_unsort3<<<g1, VEC_THREADS, 0, s>>>(c->vmu, c->perm, n_pad, d_mu);
     c->n_launches += 1;
@@ -415,10 +423,9 @@ int do_polar_energy(Ctx *c, const double *d_mu, const double *d_field, double *d
     const long long n3 = 3LL * c->n;
     int g = div_up(n3, VEC_THREADS);
     if (g > MAX_PARTIALS) g = MAX_PARTIALS;
-    double *part = c->partials + 6 * MAX_PARTIALS;
-    k_energy_partials<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, part);
-    k_energy_final<<<1, VEC_THREADS, 0, s>>>(part, g, d_energy);
-    c->n_launches += 2;
+    double *part = c->partials + 4 * (size_t)c->part_cap;
+    k_energy<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, part, c->st, d_energy);
+    c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }

@@ -54,11 +54,12 @@ __global__ void __launch_bounds__(TILE_WARPS * 32)
 k_tiles_tmu(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st,
             const typename Vec4<real>::type *__restrict__ xyzw,
             const typename Vec4<real>::type *__restrict__ mu, const double4 *__restrict__ bcentre,
-            double box, PairConsts<real> kc, double *__restrict__ acc, int n_pad) {
+            double box, PairConsts<real> kc, double *__restrict__ acc, int n_pad, int iter) {
     using vec4 = typename Vec4<real>::type;
     __shared__ vec4 s_pos[TILE_WARPS][BLOCK];
     __shared__ vec4 s_mu[TILE_WARPS][BLOCK];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     const long long n_tiles = st->n_tiles;
     const long long stride = (long long)gridDim.x * TILE_WARPS;
     for (long long t = (long long)blockIdx.x * TILE_WARPS + w; t < n_tiles; t += stride) {
@@ -131,11 +132,12 @@ __global__ void __launch_bounds__(TILE_WARPS * 32)
 k_tiles_field(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st,
               const typename Vec4<real>::type *__restrict__ xyzw,
               const typename Vec4<real>::type *__restrict__ mp, const double4 *__restrict__ bcentre,
-              double box, PairConsts<real> kc, double *__restrict__ acc, int n_pad) {
+              double box, PairConsts<real> kc, double *__restrict__ acc, int n_pad, int iter) {
     using vec4 = typename Vec4<real>::type;
     __shared__ vec4 s_pos[TILE_WARPS][BLOCK];
     __shared__ vec4 s_mp[3][TILE_WARPS][BLOCK];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     const long long n_tiles = st->n_tiles;
     const long long stride = (long long)gridDim.x * TILE_WARPS;
     for (long long t = (long long)blockIdx.x * TILE_WARPS + w; t < n_tiles; t += stride) {
@@ -217,10 +219,10 @@ static int tile_grid(Ctx *c) {
         auto k = make_consts<REAL>(p);                                                                \
         if (c->h_state->per_pair_image)                                                               \
             KERNEL<REAL, true><<<grid, TILE_WARPS * 32, 0, s>>>(c->pairs, c->st, XYZW, DATA, c->bcentre, \
-                                                                p.box, k, c->acc, c->n_pad);          \
+                                                                p.box, k, c->acc, c->n_pad, c->spec_iter);          \
         else                                                                                          \
             KERNEL<REAL, false><<<grid, TILE_WARPS * 32, 0, s>>>(c->pairs, c->st, XYZW, DATA, c->bcentre, \
-                                                                 p.box, k, c->acc, c->n_pad);         \
+                                                                 p.box, k, c->acc, c->n_pad, c->spec_iter);         \
     } while (0)
 
 int tiles_tmatvec(Ctx *c, cudaStream_t s) {

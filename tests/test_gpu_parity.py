@@ -159,6 +159,28 @@ def test_atom_mode_lists_are_exact_and_deterministic():
     small.close()
 
 
+@pytest.mark.parametrize("precision", ["mixed", "fp64"])
+@pytest.mark.parametrize("chunk", [256, 416])
+def test_atom_mode_multi_chunk_staging(precision, chunk):
+    """ATOM mode with a small shared-memory chunk: every group needs several interleaved chunks
+    (DESIGN.md 5.3); T.mu and the field still match the oracle and the list is still exact."""
+    pk = _pk()
+    s = SYSTEMS["water_6000"]()
+    P = pk.Polarizer.for_system(s, precision=pk.TKHP_FP64 if precision == "fp64" else pk.TKHP_MIXED,
+                                list_mode=pk.TKHP_LIST_ATOM, max_stage_per_chunk=chunk,
+                                max_nbrs_per_atom=512)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    n_pair, n_slots, mode = P.nblist_stats()
+    assert mode == pk.TKHP_LIST_ATOM and n_pair == oracle.count_pairs(s)
+    assert 2 * n_pair <= n_slots <= 4 * n_pair
+    rng = np.random.default_rng(5)
+    mu = rng.standard_normal((s.n_atoms, 3)) * 0.1
+    assert _rel_l2(P.tmatvec(mu).cpu().numpy(), oracle.tmatvec(s, mu)) <= TOL_VEC[precision]
+    E = P.perm_field(s.charge, s.dipole, s.quad).cpu().numpy()
+    assert _rel_l2(E, oracle.perm_field(s)) <= TOL_VEC[precision]
+    P.close()
+
+
 def test_tmatvec_symmetry_on_gpu():
     """nu.T mu == mu.T nu for the GPU operator as well (FP64 mode)."""
     import torch
