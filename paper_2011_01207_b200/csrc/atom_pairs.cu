@@ -120,7 +120,7 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         }
         int kmax = k;
         for (int o = 16; o > 0; o >>= 1) kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
-        int qmax = (kmax + 3) >> 2;
+        int qmax = ((kmax + 7) >> 3) << 1;      // even: the pair kernels take two quads per trip
         if (q0 + qmax > q_cap) {
             if (lane == 0) st->atom_bad = 1;
             qmax = q_cap - q0;
@@ -141,54 +141,129 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     }
 }
 
+// ----------------------------------------------------------------------------- bank-aware order
+// The pair kernels gather 16-byte records from shared memory, one per lane and step.  A quarter
+// warp (8 lanes) is served in one wavefront only if its 8 records fall into 8 different bank
+// groups (record index mod 8); with the lists in staging order they are random and an LDS.128
+// costs 2.35 wavefronts instead of 1 (ncu, r01).  k_atom_reorder permutes every lane's list, per
+// chunk and in place, so that at step t lane l reads a record of bank group (t + l) mod 8 whenever
+// it has one left: entries are dealt into 8 per-bank columns of rows t = ((b - l) mod 8) + 8 r;
+// entries of over-full columns (rows beyond the common padded length) move into the holes of
+// under-full ones (those steps may conflict), the remaining holes are the padding.  The set of
+// entries of a list does not change, only their order, so the result changes by FP32 summation
+// order only.  One warp per 32-atom block, list columns in shared memory ([row][lane], u16).
+constexpr int RO_ROWS = 256;          // rows per lane the shared-memory image can hold
+constexpr int RO_WARPS = 4;
+
+__global__ void __launch_bounds__(RO_WARPS * 32)
+k_atom_reorder(ClusterWs ws, int n_blocks, int rec_bytes, int s_chunk) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int blk = blockIdx.x * RO_WARPS + w;
+    if (blk >= n_blocks) return;
+    uint16_t *img = reinterpret_cast<uint16_t *>(smem_raw) + (size_t)w * RO_ROWS * 32 + lane;   // img[row * 32]
+    uint2 *__restrict__ list = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
+    const int32_t *__restrict__ arow = ws.arow + (size_t)blk * (NCH_MAX + 1);
+    const unsigned dummy = (unsigned)s_chunk * (unsigned)rec_bytes;
+    const int l8 = lane & 7;
+
+    for (int c = 0; c < NCH_MAX; ++c) {
+        const int q0 = arow[c] >> 2, q1 = arow[c + 1] >> 2;
+        const int len = (q1 - q0) << 2;                    // common padded length of this chunk's lists
+        if (len <= 0) continue;
+        if (len > RO_ROWS) continue;                       // image too small: keep staging order
+        for (int r = 0; r < RO_ROWS; ++r) img[r * 32] = 0xffffu;
+        // deal the entries into the per-bank columns
+        unsigned long long cnt = 0;                        // 8 counters of 8 bits
+        bool fits = true;
+        for (int q = q0; q < q1; ++q) {
+            const uint2 e = list[(size_t)q * 32];
+            const unsigned v[4] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16};
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                if (v[h] == dummy) continue;
+                const unsigned b = (v[h] >> 4) & 7u;
+                const unsigned r = (unsigned)(cnt >> (8 * b)) & 0xffu;
+                const unsigned t = ((b - (unsigned)l8) & 7u) + 8u * r;
+                if (t < (unsigned)RO_ROWS) img[t * 32] = (uint16_t)v[h]; else fits = false;
+                cnt += 1ull << (8 * b);
+            }
+        }
+        if (!__all_sync(0xffffffffu, fits)) continue;      // (never seen) a column ran past the image
+        // over-full columns -> holes of under-full ones
+        const unsigned R = (unsigned)len >> 3;             // rows each column keeps
+        unsigned hb = 0, hr = (unsigned)cnt & 0xffu;       // hole cursor: column hb, row hr
+        for (unsigned b = 0; b < 8; ++b) {
+            const unsigned cb = (unsigned)(cnt >> (8 * b)) & 0xffu;
+            for (unsigned r = R; r < cb; ++r) {
+                const unsigned t = ((b - (unsigned)l8) & 7u) + 8u * r;
+                const uint16_t v = img[t * 32];
+                while (hr >= R) { ++hb; hr = (unsigned)(cnt >> (8 * hb)) & 0xffu; }
+                img[(((hb - (unsigned)l8) & 7u) + 8u * hr) * 32] = v;
+                ++hr;
+            }
+        }
+        // write back; untouched holes (0xffff) are the padding
+        for (int q = q0; q < q1; ++q) {
+            unsigned v[4];
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const unsigned x = img[(((q - q0) << 2) + h) * 32];
+                v[h] = x == 0xffffu ? dummy : x;
+            }
+            list[(size_t)q * 32] = make_uint2(v[0] | (v[1] << 16), v[2] | (v[3] << 16));
+        }
+        __syncwarp();
+    }
+}
+
 // ----------------------------------------------------------------------------- pair kernels
 //   MODE_TMU   (T1,T2): out_i += -m1 mu_j + m2 (mu_j.R) R            staged: pos+w, mu
 //   MODE_FIELD (F1,F2): field at i from (q,d,Q)_j, same-group pairs contribute zero here (the FP64
 //                       correction pass adds them, pcg.cu)            staged: pos+w, 3 multipole vec4
-template <typename real, int MODE>
-__device__ __forceinline__ void eval_pair2(const unsigned char *s_base, int pay_stride, unsigned o0, unsigned o1,
+template <typename real, int MODE, int W>
+__device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_stride, const unsigned (&off)[W],
                                            const typename Vec4<real>::type &pi, real gi,
                                            const PairConsts<real> &kc, real &ax, real &ay, real &az) {
     using vec4 = typename Vec4<real>::type;
     constexpr int NK = MODE == MODE_TMU ? 2 : 3;
-    const unsigned off[2] = {o0, o1};
-    vec4 pj[2];
-    real Rx[2], Ry[2], Rz[2], r2[2], ww[2], G[2][NK];
+    vec4 pj[W];
+    real Rx[W], Ry[W], Rz[W], r2[W], ww[W], G[W][NK];
 #pragma unroll
-    for (int u = 0; u < 2; ++u) pj[u] = *reinterpret_cast<const vec4 *>(s_base + off[u]);
+    for (int u = 0; u < W; ++u) pj[u] = *reinterpret_cast<const vec4 *>(s_base + off[u]);
     if (MODE == MODE_TMU) {
-        vec4 mj[2];
+        vec4 mj[W];
 #pragma unroll
-        for (int u = 0; u < 2; ++u) mj[u] = *reinterpret_cast<const vec4 *>(s_base + pay_stride + off[u]);
+        for (int u = 0; u < W; ++u) mj[u] = *reinterpret_cast<const vec4 *>(s_base + pay_stride + off[u]);
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < W; ++u) {
             Rx[u] = pi.x - pj[u].x; Ry[u] = pi.y - pj[u].y; Rz[u] = pi.z - pj[u].z;
             r2[u] = Rx[u] * Rx[u] + Ry[u] * Ry[u] + Rz[u] * Rz[u];
             ww[u] = pi.w * pj[u].w;
         }
-        radial_w<NK, 2>(r2, ww, kc, G);
+        radial_w<NK, W>(r2, ww, kc, G);
 #pragma unroll
-        for (int u = 0; u < 2; ++u)
+        for (int u = 0; u < W; ++u)
             tmu_apply<real>(G[u][0], G[u][1], Rx[u], Ry[u], Rz[u], mj[u].x, mj[u].y, mj[u].z, ax, ay, az);
     } else {
-        vec4 b0v[2], b1v[2], b2v[2];
-        bool in[2];
+        vec4 b0v[W], b1v[W], b2v[W];
+        bool in[W];
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < W; ++u) {
             b0v[u] = *reinterpret_cast<const vec4 *>(s_base + pay_stride + off[u]);
             b1v[u] = *reinterpret_cast<const vec4 *>(s_base + 2 * pay_stride + off[u]);
             b2v[u] = *reinterpret_cast<const vec4 *>(s_base + 3 * pay_stride + off[u]);
         }
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < W; ++u) {
             Rx[u] = pi.x - pj[u].x; Ry[u] = pi.y - pj[u].y; Rz[u] = pi.z - pj[u].z;
             r2[u] = Rx[u] * Rx[u] + Ry[u] * Ry[u] + Rz[u] * Rz[u];
             ww[u] = pi.w * pj[u].w;
             in[u] = b2v[u].z != gi;
         }
-        radial_w<NK, 2>(r2, ww, kc, G);
+        radial_w<NK, W>(r2, ww, kc, G);
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
+        for (int u = 0; u < W; ++u) {
             if (!in[u]) { G[u][0] = 0; G[u][1] = 0; G[u][2] = 0; }
             field_apply<real>(G[u], Rx[u], Ry[u], Rz[u], b0v[u].x, b0v[u].y, b0v[u].z, b0v[u].w, b1v[u].x,
                               b1v[u].y, b1v[u].z, b1v[u].w, b2v[u].x, b2v[u].y, ax, ay, az);
@@ -196,8 +271,39 @@ __device__ __forceinline__ void eval_pair2(const unsigned char *s_base, int pay_
     }
 }
 
+// pairs evaluated together per lane (independent dependency chains): 4 in the FP32 T.mu kernel
+// (a 98k-atom system has only ~21 warps per SM, so the latency must be covered inside the warp),
+// 2 elsewhere (register budget)
+template <typename real, int MODE> struct PairWidth { static constexpr int W = 2; };
+template <> struct PairWidth<float, MODE_TMU> { static constexpr int W = 2; };   // 4 measured slower (80 registers)
+
+// one lane's quad of list entries (8 bytes), read-only path, pinned in program order
+__device__ __forceinline__ uint2 ldg_list(const uint2 *p) {
+    uint2 v;
+    asm volatile("ld.global.nc.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+    return v;
+}
+
 template <typename real, int MODE>
-__global__ void __launch_bounds__(GT)
+__device__ __forceinline__ void eval_quad(const unsigned char *s_base, int pay_stride, uint2 e,
+                                          const typename Vec4<real>::type &pi, real gi,
+                                          const PairConsts<real> &kc, real &ax, real &ay, real &az) {
+    if (PairWidth<real, MODE>::W == 4) {
+        const unsigned off[4] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16};
+        eval_pairs<real, MODE, 4>(s_base, pay_stride, off, pi, gi, kc, ax, ay, az);
+    } else {
+        const unsigned o0[2] = {e.x & 0xffffu, e.x >> 16}, o1[2] = {e.y & 0xffffu, e.y >> 16};
+        eval_pairs<real, MODE, 2>(s_base, pay_stride, o0, pi, gi, kc, ax, ay, az);
+        eval_pairs<real, MODE, 2>(s_base, pay_stride, o1, pi, gi, kc, ax, ay, az);
+    }
+}
+
+// resident CTAs per SM the register allocation must allow: FP32 T.mu 4 (<= 64 registers; shared
+// memory allows 4 x 56 KB), FP32 field 2 (112 KB of staging), FP64 1
+template <typename real, int MODE> struct MinCtas { static constexpr int N = sizeof(real) == 8 ? 1 : (MODE == MODE_TMU ? 3 : 2); };
+
+template <typename real, int MODE>
+__global__ void __launch_bounds__(GT, MinCtas<real, MODE>::N)
 k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
              const typename Vec4<real>::type *__restrict__ stage_pos,
              const typename Vec4<real>::type *__restrict__ data,   // mu (n_pad) or multipoles (3 n_pad)
@@ -206,6 +312,7 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     using vec4 = typename Vec4<real>::type;
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
+    constexpr int SU = 2;         // staging loads in flight per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
     vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk + 1], last = dummy
     vec4 *s_pay = s_pos + (s_chunk + 1);                       // NPAY arrays of [s_chunk + 1]
@@ -240,28 +347,53 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
 
     for (int c = 0; c < n_chunks; ++c) {
         __syncthreads();
-        for (int l = t, idx = c + t * n_chunks; idx < count; l += GT, idx += GT * n_chunks) {
-            const int a = ws.stage_atom[gbase + idx];
-            s_pos[l] = stage_pos[gbase + idx];
+        // gather of the payload by staged atom: SU records per thread in flight (index, then payload)
+        for (int l0 = t, i0 = c + t * n_chunks; i0 < count; l0 += SU * GT, i0 += SU * GT * n_chunks) {
+            int a[SU];
+            vec4 p[SU];
 #pragma unroll
-            for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + l] = data[(size_t)k * n_pad + a];
+            for (int u = 0; u < SU; ++u) {
+                const int idx = i0 + u * GT * n_chunks;
+                const bool ok = idx < count;
+                a[u] = ok ? ws.stage_atom[gbase + idx] : -1;
+                if (ok) p[u] = stage_pos[gbase + idx];
+            }
+#pragma unroll
+            for (int k = 0; k < NPAY; ++k) {
+                vec4 d[SU];
+#pragma unroll
+                for (int u = 0; u < SU; ++u)
+                    if (a[u] >= 0) d[u] = data[(size_t)k * n_pad + a[u]];
+#pragma unroll
+                for (int u = 0; u < SU; ++u)
+                    if (a[u] >= 0) s_pay[k * pstride + l0 + u * GT] = d[u];
+            }
+#pragma unroll
+            for (int u = 0; u < SU; ++u)
+                if (a[u] >= 0) s_pos[l0 + u * GT] = p[u];
         }
         __syncthreads();
         if (!active) continue;
         const int q0 = arow[c] >> 2, q1 = arow[c + 1] >> 2;
         if (q0 >= q1) continue;
         const unsigned char *s_base = smem_raw;
-        // list quads are fetched two steps ahead of their use (L2 latency under load ~ one step)
-        uint2 e = lp[(size_t)q0 * 32];
-        uint2 e1 = lp[(size_t)(q0 + 1 < q1 ? q0 + 1 : q0) * 32];
-        for (int q = q0; q < q1; ++q) {
-            const int qn = q + 2 < q1 ? q + 2 : q1 - 1;
-            const uint2 e2 = lp[(size_t)qn * 32];
-            eval_pair2<real, MODE>(s_base, pay_stride, e.x & 0xffffu, e.x >> 16, pi, gi, kc, ax, ay, az);
-            eval_pair2<real, MODE>(s_base, pay_stride, e.y & 0xffffu, e.y >> 16, pi, gi, kc, ax, ay, az);
-            e = e1;
-            e1 = e2;
-            if (++since_flush == 8) {          // every 32 entries: FP32 partial -> FP64 accumulator
+        // Two quads per trip; a quad is loaded one whole trip (8 pairs) before its use, right after
+        // the registers it goes to have been unpacked.  The loads are
+        // volatile asm so that they stay where they are written: a load that drifts to the end of
+        // the loop body shares its scoreboard with the unpack at the top and exposes the full L2
+        // latency in every trip (measured: 30 % of all stall samples).
+        const uint2 *pq = lp + (size_t)q0 * 32;
+        const uint2 *const pend = lp + (size_t)(q1 - 1) * 32;      // clamp for the look-ahead loads
+        uint2 eA = ldg_list(pq);
+        uint2 eB = ldg_list(pq + 32);
+        for (int q = q0; q < q1; q += 2, pq += 64) {
+            const uint2 a = eA;
+            eA = ldg_list(pq + 64 <= pend ? pq + 64 : pend);
+            eval_quad<real, MODE>(s_base, pay_stride, a, pi, gi, kc, ax, ay, az);
+            const uint2 b = eB;
+            eB = ldg_list(pq + 96 <= pend ? pq + 96 : pend);
+            eval_quad<real, MODE>(s_base, pay_stride, b, pi, gi, kc, ax, ay, az);
+            if (++since_flush == 4) {          // every 32 entries: FP32 partial -> FP64 accumulator
                 dx += (double)ax; dy += (double)ay; dz += (double)az;
                 ax = 0; ay = 0; az = 0;
                 since_flush = 0;
@@ -304,7 +436,14 @@ int atom_build(Ctx *c, cudaStream_t s) {
         k_atom_lists<double><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos64, ws.stage_pos64, rc2, c->st);
     else
         k_atom_lists<float><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos32, ws.stage_pos32, (float)rc2, c->st);
-    c->n_launches += 1;
+    static bool ro_configured = false;
+    const size_t ro_smem = (size_t)RO_WARPS * RO_ROWS * 32 * sizeof(uint16_t);
+    if (!ro_configured) {
+        TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_reorder, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ro_smem));
+        ro_configured = true;
+    }
+    k_atom_reorder<<<div_up(c->n_blocks, RO_WARPS), RO_WARPS * 32, ro_smem, s>>>(ws, c->n_blocks, f64 ? 32 : 16, s_chunk);
+    c->n_launches += 2;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }
