@@ -14,14 +14,17 @@
 //    arithmetic in the loop).  A lane owns one atom and only ever updates that atom: no atomics,
 //    bit-reproducible results;
 //  * entries are 16-bit BYTE OFFSETS into the staged chunk, stored per block as
-//    [entry/4][lane][entry%4]: one coalesced 8-byte load per lane fetches 4 entries, fetched one
-//    step ahead of their use;
+//    [entry/8][lane][entry%8]: 16 bytes per lane and trip of 8 pairs, a coalesced 512-byte row per
+//    warp.  The FP32 T.mu kernel streams the rows through a per-warp shared-memory ring with
+//    cp.async, several trips ahead (the L2/HBM latency of this stream was the largest stall of
+//    the register-prefetch version); the other variants load them one trip ahead into registers;
 //  * the loss of coalescing the paper notes becomes per-lane LDS.128 gathers from shared memory;
 //    two pairs are evaluated together per lane (two independent dependency chains);
 //  * FP32 partial sums are flushed into FP64 registers every 32 entries.
 // The lists are built from the CLUSTER lists (the 8-atom-cluster list is the candidate set of
 // each of its atoms): k_atom_lists below.
 #include "cluster.cuh"
+#include "f32x2.cuh"
 #include "reduce.cuh"
 
 namespace tkhp {
@@ -47,6 +50,9 @@ struct PcgFuse {
 // ITS atom to its own list; the warp then pads all 32 lists of the chunk to a common length
 // (multiple of 4).  The test is the pair kernels' own arithmetic (group-frame coordinates, FP32 in
 // MIXED, FP64 in FP64 mode).
+// quad q (4 entries) of a lane, as uint2 index relative to the lane's first quad (lane * 2)
+__host__ __device__ __forceinline__ size_t qidx(int q) { return (size_t)(q >> 1) * 64 + (size_t)(q & 1); }
+
 template <typename real>
 __global__ void __launch_bounds__(GT)
 k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
@@ -73,8 +79,8 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int oct = slot >> 3;
     const int L = active ? ws.oct_len[oct] : 0;
     const uint16_t *__restrict__ ent = ws.entries + (size_t)oct * ws.l_cap;
-    // a lane's list as quads of 4 entries: quad q of lane l at uint2 index q * 32 + l of the block
-    uint2 *__restrict__ out = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
+    // a lane's list as quads of 4 entries: quad q of lane l at uint2 index qidx(q) + 2 l of the block
+    uint2 *__restrict__ out = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane * 2;
     int32_t *__restrict__ arow = ws.arow + (size_t)blk * (NCH_MAX + 1);
     const unsigned dummy = (unsigned)s_chunk * (unsigned)sizeof(vec4);
     const unsigned long long dummy4 = 0x0001000100010001ull * (unsigned long long)dummy;
@@ -111,7 +117,7 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
                     pend |= (unsigned long long)(loc * (unsigned)sizeof(vec4)) << ((k & 3) * 16);
                     if ((k & 3) == 3) {
                         const int q = q0 + (k >> 2);
-                        if (q < q_cap) out[(size_t)q * 32] = make_uint2((unsigned)pend, (unsigned)(pend >> 32));
+                        if (q < q_cap) out[qidx(q)] = make_uint2((unsigned)pend, (unsigned)(pend >> 32));
                         pend = 0;
                     }
                     ++k;
@@ -128,10 +134,10 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         int qd = k >> 2;                   // first quad this lane has not stored yet
         if ((k & 3) != 0) {                // partly filled quad: the rest are dummies
             pend |= dummy4 << ((k & 3) * 16);
-            if (q0 + qd < q_cap) out[(size_t)(q0 + qd) * 32] = make_uint2((unsigned)pend, (unsigned)(pend >> 32));
+            if (q0 + qd < q_cap) out[qidx(q0 + qd)] = make_uint2((unsigned)pend, (unsigned)(pend >> 32));
             ++qd;
         }
-        for (; qd < qmax; ++qd) out[(size_t)(q0 + qd) * 32] = make_uint2((unsigned)dummy4, (unsigned)(dummy4 >> 32));
+        for (; qd < qmax; ++qd) out[qidx(q0 + qd)] = make_uint2((unsigned)dummy4, (unsigned)(dummy4 >> 32));
         q0 += qmax;
     }
     const int k0 = q0 << 2;
@@ -162,7 +168,7 @@ k_atom_reorder(ClusterWs ws, int n_blocks, int rec_bytes, int s_chunk) {
     const int blk = blockIdx.x * RO_WARPS + w;
     if (blk >= n_blocks) return;
     uint16_t *img = reinterpret_cast<uint16_t *>(smem_raw) + (size_t)w * RO_ROWS * 32 + lane;   // img[row * 32]
-    uint2 *__restrict__ list = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
+    uint2 *__restrict__ list = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane * 2;
     const int32_t *__restrict__ arow = ws.arow + (size_t)blk * (NCH_MAX + 1);
     const unsigned dummy = (unsigned)s_chunk * (unsigned)rec_bytes;
     const int l8 = lane & 7;
@@ -177,7 +183,7 @@ k_atom_reorder(ClusterWs ws, int n_blocks, int rec_bytes, int s_chunk) {
         unsigned long long cnt = 0;                        // 8 counters of 8 bits
         bool fits = true;
         for (int q = q0; q < q1; ++q) {
-            const uint2 e = list[(size_t)q * 32];
+            const uint2 e = list[qidx(q)];
             const unsigned v[4] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16};
 #pragma unroll
             for (int h = 0; h < 4; ++h) {
@@ -211,7 +217,7 @@ k_atom_reorder(ClusterWs ws, int n_blocks, int rec_bytes, int s_chunk) {
                 const unsigned x = img[(((q - q0) << 2) + h) * 32];
                 v[h] = x == 0xffffu ? dummy : x;
             }
-            list[(size_t)q * 32] = make_uint2(v[0] | (v[1] << 16), v[2] | (v[3] << 16));
+            list[qidx(q)] = make_uint2(v[0] | (v[1] << 16), v[2] | (v[3] << 16));
         }
         __syncwarp();
     }
@@ -221,12 +227,99 @@ k_atom_reorder(ClusterWs ws, int n_blocks, int rec_bytes, int s_chunk) {
 //   MODE_TMU   (T1,T2): out_i += -m1 mu_j + m2 (mu_j.R) R            staged: pos+w, mu
 //   MODE_FIELD (F1,F2): field at i from (q,d,Q)_j, same-group pairs contribute zero here (the FP64
 //                       correction pass adds them, pcg.cu)            staged: pos+w, 3 multipole vec4
+// ---- FP32 partial sums of one lane ------------------------------------------------------------
+// Generic: one (x, y, z) partial.  Packed FP32 T.mu: two partials, C = sum G2/3 (mu_j.D) D and
+// M = sum G1 mu_j (D = r_j - r_i), so that the pair loop needs neither the factor 3 nor a
+// negation; (T mu)_i = 3 C - M is formed at every flush into the FP64 registers.
+template <typename real, int MODE>
+struct Partial {
+    real x = 0, y = 0, z = 0;
+    __device__ __forceinline__ void flush(double &dx, double &dy, double &dz) {
+        dx += (double)x; dy += (double)y; dz += (double)z;
+        x = 0; y = 0; z = 0;
+    }
+};
+template <>
+struct Partial<float, MODE_TMU> {
+    f2 cxy = 0ull, mxy = 0ull;
+    float cz = 0.f, mz = 0.f;
+    __device__ __forceinline__ void flush(double &dx, double &dy, double &dz) {
+        dx += (double)fmaf(3.0f, lo(cxy), -lo(mxy));
+        dy += (double)fmaf(3.0f, hi(cxy), -hi(mxy));
+        dz += (double)fmaf(3.0f, cz, -mz);
+        cxy = 0ull; mxy = 0ull; cz = 0.f; mz = 0.f;
+    }
+};
+
+// ---- packed FP32 T.mu: two list entries of one lane per call ------------------------------------
+// The two pairs (j0, j1) of a lane share every instruction of the radial chain (lo half = j0,
+// hi half = j1); the geometry and the 3-vector updates are packed over (x, y), the pair LDS.128
+// delivers them in.  Per pair: 25 FMA-pipe issue slots (41 pipe cycles) + 4 MUFU, against 46
+// scalar instructions.  Per-lane constants: pxy = (x_i, y_i), nz0 = (-z_i, 0),
+// one_w = (1, w_i log2 e) so that one FFMA2 gives (z_j - z_i, w_i w_j log2 e).
+struct TmuLane {
+    f2 pxy, nz0, one_w;
+};
+struct TmuConsts {
+    float pb;       // 0.4 beta:              u = 1 / (1 + pb R)
+    float nb2l;     // -beta^2 log2 e:        e^{-z^2} = ex2(nb2l R^2)
+    float c1b;      // (2/sqrt pi) beta:      c z
+    float k3;       // (4/(3 sqrt pi)) beta^3: (2c/3) z^3 = k3 R^3
+};
+
+__device__ __forceinline__ void tmu_pair2(const unsigned char *s_base, int pay_stride, unsigned off0, unsigned off1,
+                                          const TmuLane &L, const TmuConsts &K, Partial<float, MODE_TMU> &A) {
+    constexpr float c[TKHP_ERFCX_DEG + 1] = TKHP_ERFCX_COEFFS;
+    constexpr float LN2 = 0.69314718055994531f;
+    const ulonglong2 p0 = *reinterpret_cast<const ulonglong2 *>(s_base + off0);               // (x,y) (z,w)
+    const ulonglong2 p1 = *reinterpret_cast<const ulonglong2 *>(s_base + off1);
+    const ulonglong2 m0 = *reinterpret_cast<const ulonglong2 *>(s_base + pay_stride + off0);  // (mx,my) (mz,0)
+    const ulonglong2 m1 = *reinterpret_cast<const ulonglong2 *>(s_base + pay_stride + off1);
+    const f2 Dxy0 = sub2(p0.x, L.pxy), Dxy1 = sub2(p1.x, L.pxy);
+    const f2 Dzw0 = fma2(p0.y, L.one_w, L.nz0), Dzw1 = fma2(p1.y, L.one_w, L.nz0);
+    float s0 = lo(Dxy0) * lo(Dxy0), s1 = lo(Dxy1) * lo(Dxy1);
+    s0 = fmaf(hi(Dxy0), hi(Dxy0), s0); s1 = fmaf(hi(Dxy1), hi(Dxy1), s1);
+    s0 = fmaf(lo(Dzw0), lo(Dzw0), s0); s1 = fmaf(lo(Dzw1), lo(Dzw1), s1);
+    const f2 r2 = pk(s0, s1);
+    const f2 rinv = pk(fast_rsqrt(s0), fast_rsqrt(s1));
+    const f2 r = mul2(r2, rinv);
+    const f2 ua = fma2(r, bc(K.pb), bc(1.0f));
+    const f2 u = pk(fast_rcp(lo(ua)), fast_rcp(hi(ua)));
+    const f2 ea = mul2(r2, bc(K.nb2l));
+    const f2 ez = pk(fast_ex2(lo(ea)), fast_ex2(hi(ea)));
+    const f2 r3 = mul2(r2, r);
+    const f2 xl = pk(lo(r3) * hi(Dzw0), hi(r3) * hi(Dzw1));         // x log2 e
+    const f2 et = pk(fast_ex2(-lo(xl)), fast_ex2(-hi(xl)));
+    f2 p = bc(c[TKHP_ERFCX_DEG]);
+#pragma unroll
+    for (int d = TKHP_ERFCX_DEG - 1; d >= 0; --d) p = fma2(p, u, bc(c[d]));
+    const f2 g1 = fma2(r, bc(K.c1b), p);                             // erfcx(z) + c z
+    const f2 a1 = fma2(ez, g1, neg2(et));                            // R^3 G1
+    const f2 h2 = fma2(r3, bc(K.k3), g1);
+    const f2 x = mul2(xl, bc(LN2));
+    const f2 xe = fma2(x, et, et);                                   // (1 + x) e^-x
+    const f2 b2 = fma2(ez, h2, neg2(xe));                            // R^5 G2 / 3
+    const f2 rinv2 = mul2(rinv, rinv);
+    const f2 rinv3 = mul2(rinv2, rinv);
+    const f2 G1 = mul2(a1, rinv3);
+    const f2 G2 = mul2(b2, mul2(rinv2, rinv3));                      // G2 / 3
+    float d0 = lo(m0.x) * lo(Dxy0), d1 = lo(m1.x) * lo(Dxy1);
+    d0 = fmaf(hi(m0.x), hi(Dxy0), d0); d1 = fmaf(hi(m1.x), hi(Dxy1), d1);
+    d0 = fmaf(lo(m0.y), lo(Dzw0), d0); d1 = fmaf(lo(m1.y), lo(Dzw1), d1);
+    const f2 cc = mul2(G2, pk(d0, d1));
+    A.cxy = fma2(Dxy0, bc(lo(cc)), A.cxy); A.cz = fmaf(lo(cc), lo(Dzw0), A.cz);
+    A.mxy = fma2(m0.x, bc(lo(G1)), A.mxy); A.mz = fmaf(lo(G1), lo(m0.y), A.mz);
+    A.cxy = fma2(Dxy1, bc(hi(cc)), A.cxy); A.cz = fmaf(hi(cc), lo(Dzw1), A.cz);
+    A.mxy = fma2(m1.x, bc(hi(G1)), A.mxy); A.mz = fmaf(hi(G1), lo(m1.y), A.mz);
+}
+
 template <typename real, int MODE, int W>
 __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_stride, const unsigned (&off)[W],
                                            const typename Vec4<real>::type &pi, real gi,
-                                           const PairConsts<real> &kc, real &ax, real &ay, real &az) {
+                                           const PairConsts<real> &kc, Partial<real, MODE> &A) {
     using vec4 = typename Vec4<real>::type;
     constexpr int NK = MODE == MODE_TMU ? 2 : 3;
+    real &ax = A.x, &ay = A.y, &az = A.z;
     vec4 pj[W];
     real Rx[W], Ry[W], Rz[W], r2[W], ww[W], G[W][NK];
 #pragma unroll
@@ -284,18 +377,77 @@ __device__ __forceinline__ uint2 ldg_list(const uint2 *p) {
     return v;
 }
 
+// per-lane constants of the pair loop
+template <typename real, int MODE>
+struct LaneCtx {
+    typename Vec4<real>::type pi;
+    real gi;
+    PairConsts<real> kc;
+};
+template <>
+struct LaneCtx<float, MODE_TMU> {
+    TmuLane L;
+    TmuConsts K;
+};
+
 template <typename real, int MODE>
 __device__ __forceinline__ void eval_quad(const unsigned char *s_base, int pay_stride, uint2 e,
-                                          const typename Vec4<real>::type &pi, real gi,
-                                          const PairConsts<real> &kc, real &ax, real &ay, real &az) {
+                                          const LaneCtx<real, MODE> &lc, Partial<real, MODE> &A) {
     if (PairWidth<real, MODE>::W == 4) {
         const unsigned off[4] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16};
-        eval_pairs<real, MODE, 4>(s_base, pay_stride, off, pi, gi, kc, ax, ay, az);
+        eval_pairs<real, MODE, 4>(s_base, pay_stride, off, lc.pi, lc.gi, lc.kc, A);
     } else {
         const unsigned o0[2] = {e.x & 0xffffu, e.x >> 16}, o1[2] = {e.y & 0xffffu, e.y >> 16};
-        eval_pairs<real, MODE, 2>(s_base, pay_stride, o0, pi, gi, kc, ax, ay, az);
-        eval_pairs<real, MODE, 2>(s_base, pay_stride, o1, pi, gi, kc, ax, ay, az);
+        eval_pairs<real, MODE, 2>(s_base, pay_stride, o0, lc.pi, lc.gi, lc.kc, A);
+        eval_pairs<real, MODE, 2>(s_base, pay_stride, o1, lc.pi, lc.gi, lc.kc, A);
     }
+}
+template <>
+__device__ __forceinline__ void eval_quad<float, MODE_TMU>(const unsigned char *s_base, int pay_stride, uint2 e,
+                                                           const LaneCtx<float, MODE_TMU> &lc,
+                                                           Partial<float, MODE_TMU> &A) {
+    tmu_pair2(s_base, pay_stride, e.x & 0xffffu, e.x >> 16, lc.L, lc.K, A);
+    tmu_pair2(s_base, pay_stride, e.y & 0xffffu, e.y >> 16, lc.L, lc.K, A);
+}
+
+template <typename real, int MODE>
+__device__ __forceinline__ void make_lane(LaneCtx<real, MODE> &lc, const typename Vec4<real>::type &pi, real gi,
+                                          const PairConsts<real> &kc) {
+    lc.pi = pi; lc.gi = gi; lc.kc = kc;
+}
+template <>
+__device__ __forceinline__ void make_lane<float, MODE_TMU>(LaneCtx<float, MODE_TMU> &lc, const float4 &pi, float,
+                                                           const PairConsts<float> &kc) {
+    lc.L.pxy = pk(pi.x, pi.y);
+    lc.L.nz0 = pk(-pi.z, 0.0f);
+    lc.L.one_w = pk(1.0f, pi.w * 1.4426950408889634f);
+    lc.K.pb = kc.pb;
+    lc.K.nb2l = kc.nb2l;
+    lc.K.c1b = kc.c1b;
+    lc.K.k3 = kc.k3;
+}
+
+// trips of list rows (512 B per warp) the shared-memory ring holds; 0 = register prefetch
+template <typename real, int MODE> struct ListRing { static constexpr int N = 0; };
+template <> struct ListRing<float, MODE_TMU> { static constexpr int N = 4; };
+constexpr int RING_ROW = 512;        // bytes per warp and trip
+
+__device__ __forceinline__ void cp_async16(unsigned dst, const void *src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+template <int BYTES>
+__device__ __forceinline__ void cp_async_rec(void *dst, const void *src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
+#pragma unroll
+    for (int o = 0; o < BYTES; o += 16) cp_async16(d + o, reinterpret_cast<const unsigned char *>(src) + o);
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ uint4 lds128(unsigned addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
 }
 
 // resident CTAs per SM the register allocation must allow: FP32 T.mu 4 (<= 64 registers; shared
@@ -312,7 +464,7 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     using vec4 = typename Vec4<real>::type;
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
-    constexpr int SU = 2;         // staging loads in flight per thread
+    constexpr int SU = sizeof(real) == 8 ? 4 : 8;   // staged records in flight per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
     vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk + 1], last = dummy
     vec4 *s_pay = s_pos + (s_chunk + 1);                       // NPAY arrays of [s_chunk + 1]
@@ -330,11 +482,14 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const vec4 pi = gpos[slot];
     real gi = 0;
     if (MODE == MODE_FIELD) gi = data[2 * (size_t)n_pad + slot].z;
-    const uint2 *__restrict__ lp = reinterpret_cast<const uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
+    const uint2 *__restrict__ lp = reinterpret_cast<const uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane * 2;
     const int32_t *__restrict__ arow = ws.arow + (size_t)blk * (NCH_MAX + 1);
+    constexpr int RING = ListRing<real, MODE>::N;
 
     double dx = 0.0, dy = 0.0, dz = 0.0;
-    real ax = 0, ay = 0, az = 0;
+    Partial<real, MODE> A;
+    LaneCtx<real, MODE> lc;
+    make_lane<real, MODE>(lc, pi, gi, kc);
     int since_flush = 0;
 
     if (t == 0) {                              // permanent dummy record: far away, zero payload
@@ -345,62 +500,91 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + s_chunk] = zero;
     }
 
+    // list ring (RING > 0): the block's rows are one contiguous stream over all chunks; row tg goes
+    // to slot tg % RING of this warp's ring, RING - 1 trips before its use.  Every lane copies and
+    // reads only its own 16 bytes, so cp.async.wait_group is all the synchronisation needed.
+    const int t_total = (active && n_chunks <= NCH_MAX) ? arow[n_chunks] >> 3 : 0;
+    const uint4 *const rows = reinterpret_cast<const uint4 *>(lp);          // row tg of this lane: rows[tg * 32]
+    unsigned ring = 0;
+    int t_issue = 0;
+    if (RING > 0) {
+        ring = (unsigned)__cvta_generic_to_shared(smem_raw) + (unsigned)((1 + NPAY) * pay_stride) +
+               (unsigned)(w * RING * RING_ROW + lane * 16);
+#pragma unroll
+        for (int k = 0; k < RING - 1; ++k) {
+            if (t_issue < t_total) cp_async16(ring + (t_issue % RING) * RING_ROW, rows + (size_t)t_issue * 32);
+            cp_async_commit();
+            ++t_issue;
+        }
+    }
+
     for (int c = 0; c < n_chunks; ++c) {
         __syncthreads();
-        // gather of the payload by staged atom: SU records per thread in flight (index, then payload)
+        // staging of chunk c with cp.async (global -> shared without a register round trip): the
+        // positions do not depend on the atom index, so a thread has its index loads and position
+        // copies of up to SU records in flight together, then the payload copies by index.
         for (int l0 = t, i0 = c + t * n_chunks; i0 < count; l0 += SU * GT, i0 += SU * GT * n_chunks) {
             int a[SU];
-            vec4 p[SU];
 #pragma unroll
             for (int u = 0; u < SU; ++u) {
                 const int idx = i0 + u * GT * n_chunks;
-                const bool ok = idx < count;
-                a[u] = ok ? ws.stage_atom[gbase + idx] : -1;
-                if (ok) p[u] = stage_pos[gbase + idx];
+                a[u] = idx < count ? ws.stage_atom[gbase + idx] : -1;
+            }
+#pragma unroll
+            for (int u = 0; u < SU; ++u) {
+                const int idx = i0 + u * GT * n_chunks;
+                if (idx < count) cp_async_rec<sizeof(vec4)>(s_pos + l0 + u * GT, stage_pos + gbase + idx);
             }
 #pragma unroll
             for (int k = 0; k < NPAY; ++k) {
-                vec4 d[SU];
 #pragma unroll
                 for (int u = 0; u < SU; ++u)
-                    if (a[u] >= 0) d[u] = data[(size_t)k * n_pad + a[u]];
-#pragma unroll
-                for (int u = 0; u < SU; ++u)
-                    if (a[u] >= 0) s_pay[k * pstride + l0 + u * GT] = d[u];
+                    if (a[u] >= 0) cp_async_rec<sizeof(vec4)>(s_pay + k * pstride + l0 + u * GT, data + (size_t)k * n_pad + a[u]);
             }
-#pragma unroll
-            for (int u = 0; u < SU; ++u)
-                if (a[u] >= 0) s_pos[l0 + u * GT] = p[u];
         }
+        cp_async_commit();
+        cp_async_wait<0>();
         __syncthreads();
         if (!active) continue;
         const int q0 = arow[c] >> 2, q1 = arow[c + 1] >> 2;
         if (q0 >= q1) continue;
         const unsigned char *s_base = smem_raw;
-        // Two quads per trip; a quad is loaded one whole trip (8 pairs) before its use, right after
-        // the registers it goes to have been unpacked.  The loads are
-        // volatile asm so that they stay where they are written: a load that drifts to the end of
-        // the loop body shares its scoreboard with the unpack at the top and exposes the full L2
-        // latency in every trip (measured: 30 % of all stall samples).
-        const uint2 *pq = lp + (size_t)q0 * 32;
-        const uint2 *const pend = lp + (size_t)(q1 - 1) * 32;      // clamp for the look-ahead loads
-        uint2 eA = ldg_list(pq);
-        uint2 eB = ldg_list(pq + 32);
-        for (int q = q0; q < q1; q += 2, pq += 64) {
-            const uint2 a = eA;
-            eA = ldg_list(pq + 64 <= pend ? pq + 64 : pend);
-            eval_quad<real, MODE>(s_base, pay_stride, a, pi, gi, kc, ax, ay, az);
-            const uint2 b = eB;
-            eB = ldg_list(pq + 96 <= pend ? pq + 96 : pend);
-            eval_quad<real, MODE>(s_base, pay_stride, b, pi, gi, kc, ax, ay, az);
-            if (++since_flush == 4) {          // every 32 entries: FP32 partial -> FP64 accumulator
-                dx += (double)ax; dy += (double)ay; dz += (double)az;
-                ax = 0; ay = 0; az = 0;
-                since_flush = 0;
+        if (RING > 0) {
+            for (int tg = q0 >> 1; tg < (q1 >> 1); ++tg) {
+                if (t_issue < t_total) cp_async16(ring + (t_issue % RING) * RING_ROW, rows + (size_t)t_issue * 32);
+                cp_async_commit();
+                ++t_issue;
+                cp_async_wait<(RING > 0 ? RING - 1 : 0)>();
+                const uint4 e = lds128(ring + (tg % RING) * RING_ROW);
+                eval_quad<real, MODE>(s_base, pay_stride, make_uint2(e.x, e.y), lc, A);
+                eval_quad<real, MODE>(s_base, pay_stride, make_uint2(e.z, e.w), lc, A);
+                if ((tg & 3) == 3) A.flush(dx, dy, dz);      // every 32 entries: FP32 partial -> FP64
+            }
+        } else {
+            // Two quads per trip; a quad is loaded one whole trip (8 pairs) before its use, right after
+            // the registers it goes to have been unpacked.  The loads are volatile asm so that they
+            // stay where they are written: a load that drifts to the end of the loop body shares its
+            // scoreboard with the unpack at the top and exposes the full L2 latency in every trip.
+            const uint2 *pq = lp + qidx(q0);
+            const uint2 *const pend = lp + qidx(q1 - 2);           // clamp for the look-ahead loads
+            uint2 eA = ldg_list(pq);
+            uint2 eB = ldg_list(pq + 1);
+            for (int q = q0; q < q1; q += 2, pq += 64) {
+                const uint2 a = eA;
+                eA = ldg_list(pq + 64 <= pend ? pq + 64 : pend);
+                eval_quad<real, MODE>(s_base, pay_stride, a, lc, A);
+                const uint2 b = eB;
+                eB = ldg_list(pq + 64 <= pend ? pq + 65 : pend + 1);
+                eval_quad<real, MODE>(s_base, pay_stride, b, lc, A);
+                if (++since_flush == 4) {          // every 32 entries: FP32 partial -> FP64 accumulator
+                    A.flush(dx, dy, dz);
+                    since_flush = 0;
+                }
             }
         }
     }
-    dx += (double)ax; dy += (double)ay; dz += (double)az;
+    if (RING > 0) cp_async_wait<0>();
+    A.flush(dx, dy, dz);
     if (active) {
         acc[slot] = dx;
         acc[n_pad + slot] = dy;
@@ -454,11 +638,12 @@ static int launch_atom_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
     constexpr int which = sizeof(real) == 8;
     const int s_chunk = atom_chunk_capacity(which, ws.chunk_cap);
-    const size_t smem = sizeof(vec4) * (size_t)(1 + NPAY) * (size_t)(s_chunk + 1);
+    const size_t smem = sizeof(vec4) * (size_t)(1 + NPAY) * (size_t)(s_chunk + 1) +
+                        (size_t)ListRing<real, MODE>::N * RING_ROW * GB;
     static bool configured[2][2] = {{false, false}, {false, false}};
     if (!configured[which][MODE]) {
         TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_pairs<real, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          2 * ATOM_SMEM + 4096));
+                                          2 * ATOM_SMEM + 4096 + ListRing<real, MODE>::N * RING_ROW * GB));
         configured[which][MODE] = true;
     }
     PairConsts<real> k;
@@ -468,6 +653,13 @@ static int launch_atom_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     k.rc2 = (real)(c->p.cutoff * c->p.cutoff);
     k.box = (real)1;
     k.inv_box = (real)0;
+    {
+        const double b = c->p.ewald_beta;
+        k.pb = (real)((double)TKHP_ERFCX_P * b);
+        k.nb2l = (real)(-1.4426950408889634 * b * b);
+        k.c1b = (real)(2.0 / SQRT_PI * b);
+        k.k3 = (real)(4.0 / (3.0 * SQRT_PI) * b * b * b);
+    }
     PcgFuse fuse;
     fuse.on = MODE == MODE_TMU && c->fuse_q;
     fuse.self = 4.0 * c->p.ewald_beta * c->p.ewald_beta * c->p.ewald_beta / (3.0 * SQRT_PI);

@@ -169,7 +169,7 @@ static int launch_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
                                           SMEM_BUDGET + 1024));
         configured[which][MODE] = true;
     }
-    PairConsts<real> k;
+    PairConsts<real> k = {};
     k.beta = (real)c->p.ewald_beta;
     k.c1 = (real)(2.0 / SQRT_PI);
     k.c23 = (real)(4.0 / (3.0 * SQRT_PI));

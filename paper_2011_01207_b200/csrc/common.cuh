@@ -82,7 +82,7 @@ struct Ctx {
     uint32_t *grp_start;    // N + 1
     int32_t *grp_members;   // N
     // sorted, block-local structure of arrays
-    float4 *xyzw32;         // n_pad: local x,y,z (A), w = (a/alpha)^(1/6)
+    float4 *xyzw32;         // n_pad: local x,y,z (A), w = (a/alpha)^(1/2)
     double4 *xyzw64;        // n_pad (FP64 mode)
     double4 *bcentre;       // n_blocks: block box centre (x,y,z, 0)
     double4 *bhalf;         // n_blocks: half extent

@@ -332,7 +332,7 @@ __global__ void k_gather_blocks(const double *__restrict__ pos, const double *__
         lx = w[0] - ctr[0];
         ly = w[1] - ctr[1];
         lz = w[2] - ctr[2];
-        wf = (al > 0.0) ? pow(thole_a / al, 1.0 / 6.0) : 0.0;
+        wf = (al > 0.0) ? sqrt(thole_a / al) : 0.0;      // w = (a/alpha)^(1/2): a u^3 = R^3 w_i w_j
     } else {
         // phantom atoms: far away and mutually distant, so the cutoff test removes them
         lx = ly = lz = (double)PHANTOM_FAR * (double)(1 + lane);

@@ -3,7 +3,7 @@
 // The paper prints no interaction formula (refs only); these functions
 // implement DESIGN.md section 2 (= SURVEY 8(c)):
 //   Ewald   bn_0 = erfc(bR)/R,  bn_k = [(2k-1) bn_{k-1} + (2b^2)^k/(b sqrt(pi)) exp(-b^2R^2)]/R^2
-//   Thole   x = a R^3/sqrt(alpha_i alpha_j) = (R w_i w_j)^3, w = (a/alpha)^(1/6)
+//   Thole   x = a R^3/sqrt(alpha_i alpha_j) = R^3 w_i w_j, w = (a/alpha)^(1/2)
 //           1-lam3 = e^-x, 1-lam5 = (1+x)e^-x, 1-lam7 = (1+x+0.6x^2)e^-x
 //   (F1)    G_k = bn_k - (1 - lam_{2k+1}) rr_k        (unmasked pairs; masked pairs: correction pass)
 //   (F2)    E_i += [q_j G1 + G2 (d_j.R) + (G3/3)(R.Q_j R)] R - G1 d_j - (2/3) G2 (Q_j R)
@@ -31,6 +31,11 @@ struct PairConsts {
     real rc2;       // cutoff^2
     real box;       // box edge (PPI kernels)
     real inv_box;
+    // products formed once on the host for the packed FP32 kernels (atom_pairs.cu)
+    real pb;        // 0.4 beta:                u = 1 / (1 + pb R)
+    real nb2l;      // -beta^2 log2 e:          e^{-z^2} = ex2(nb2l R^2)
+    real c1b;       // (2/sqrt pi) beta:        c z = c1b R
+    real k3;        // (4/(3 sqrt pi)) beta^3:  (2c/3) z^3 = k3 R^3
 };
 
 template <typename real> struct Vec4;
@@ -83,9 +88,9 @@ __device__ __forceinline__ void radial_f32_w(const float (&r2)[W], const float (
 #pragma unroll
     for (int i = 0; i < W; ++i) u[i] = fast_rcp(fmaf(TKHP_ERFCX_P, z[i], 1.0f));
 #pragma unroll
-    for (int i = 0; i < W; ++i) { z2[i] = z[i] * z[i]; t[i] = r[i] * ww[i]; }
+    for (int i = 0; i < W; ++i) { z2[i] = z[i] * z[i]; t[i] = r2[i] * r[i]; }
 #pragma unroll
-    for (int i = 0; i < W; ++i) { ez[i] = fast_ex2(z2[i] * NLOG2E); x[i] = t[i] * t[i] * t[i]; }
+    for (int i = 0; i < W; ++i) { ez[i] = fast_ex2(z2[i] * NLOG2E); x[i] = t[i] * ww[i]; }
 #pragma unroll
     for (int i = 0; i < W; ++i) { et[i] = fast_ex2(x[i] * NLOG2E); p[i] = c[TKHP_ERFCX_DEG]; }
 #pragma unroll
@@ -139,8 +144,7 @@ __device__ __forceinline__ void radial_f64(double r2, double ww, const PairConst
     const double cz = k.c1 * z;
     const double z2 = z * z;
     const double B1 = erfc(z) + cz * ez;
-    const double t = r * ww;
-    const double x = t * t * t;
+    const double x = (r2 * r) * ww;
     const double et = exp(-x);
     const double rinv3 = rinv2 * rinv;
     G[0] = (B1 - et) * rinv3;

@@ -195,7 +195,7 @@ k_tiles_field(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st
 
 template <typename real>
 static PairConsts<real> make_consts(const tkhp_params &p) {
-    PairConsts<real> k;
+    PairConsts<real> k = {};
     k.beta = (real)p.ewald_beta;
     k.c1 = (real)(2.0 / SQRT_PI);
     k.c23 = (real)(4.0 / (3.0 * SQRT_PI));
