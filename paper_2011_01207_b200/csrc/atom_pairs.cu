@@ -476,8 +476,13 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int count = ws.stage_count[g];
     const int n_chunks = atom_chunks_of(count, s_chunk);
     const size_t gbase = (size_t)g * ws.s_cap;
-    const bool active = w < nb;
-    const int blk = b0 + (active ? w : 0);
+    // warps per block: a group with few blocks (small systems: config 1 has 1.7 blocks per group)
+    // gives each block to 2, 4 or 8 warps; warp `part` of a block takes the block's list rows
+    // part, part + wpb, ... and the parts are added in a fixed order at the end (bit-reproducible)
+    const int wpb = nb >= 5 ? 1 : (nb >= 3 ? 2 : (nb == 2 ? 4 : 8));
+    const int kb = w / wpb, part = w - kb * wpb;
+    const bool active = kb < nb;
+    const int blk = b0 + (active ? kb : 0);
     const int slot = blk * BLOCK + lane;
     const vec4 pi = gpos[slot];
     real gi = 0;
@@ -500,21 +505,22 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + s_chunk] = zero;
     }
 
-    // list ring (RING > 0): the block's rows are one contiguous stream over all chunks; row tg goes
-    // to slot tg % RING of this warp's ring, RING - 1 trips before its use.  Every lane copies and
-    // reads only its own 16 bytes, so cp.async.wait_group is all the synchronisation needed.
+    // list ring (RING > 0): the block's rows are one contiguous stream over all chunks; this warp's
+    // m-th row (row part + m wpb) goes to slot m % RING of its ring, RING - 1 trips before its use.
+    // Every lane copies and reads only its own 16 bytes, so cp.async.wait_group is all the
+    // synchronisation needed.
     const int t_total = (active && n_chunks <= NCH_MAX) ? arow[n_chunks] >> 3 : 0;
     const uint4 *const rows = reinterpret_cast<const uint4 *>(lp);          // row tg of this lane: rows[tg * 32]
     unsigned ring = 0;
-    int t_issue = 0;
+    int t_issue = part, m_issue = 0, m_use = 0;
     if (RING > 0) {
         ring = (unsigned)__cvta_generic_to_shared(smem_raw) + (unsigned)((1 + NPAY) * pay_stride) +
                (unsigned)(w * RING * RING_ROW + lane * 16);
 #pragma unroll
         for (int k = 0; k < RING - 1; ++k) {
-            if (t_issue < t_total) cp_async16(ring + (t_issue % RING) * RING_ROW, rows + (size_t)t_issue * 32);
+            if (t_issue < t_total) cp_async16(ring + (m_issue % RING) * RING_ROW, rows + (size_t)t_issue * 32);
             cp_async_commit();
-            ++t_issue;
+            t_issue += wpb; ++m_issue;
         }
     }
 
@@ -550,31 +556,39 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         if (q0 >= q1) continue;
         const unsigned char *s_base = smem_raw;
         if (RING > 0) {
-            for (int tg = q0 >> 1; tg < (q1 >> 1); ++tg) {
-                if (t_issue < t_total) cp_async16(ring + (t_issue % RING) * RING_ROW, rows + (size_t)t_issue * 32);
+            // my rows of this chunk: the smallest tg >= first row with tg = part (mod wpb)
+            const int r0 = q0 >> 1;
+            for (int tg = r0 + ((part - r0) & (wpb - 1)); tg < (q1 >> 1); tg += wpb) {
+                if (t_issue < t_total) cp_async16(ring + (m_issue % RING) * RING_ROW, rows + (size_t)t_issue * 32);
                 cp_async_commit();
-                ++t_issue;
+                t_issue += wpb; ++m_issue;
                 cp_async_wait<(RING > 0 ? RING - 1 : 0)>();
-                const uint4 e = lds128(ring + (tg % RING) * RING_ROW);
+                const uint4 e = lds128(ring + (m_use % RING) * RING_ROW);
+                ++m_use;
                 eval_quad<real, MODE>(s_base, pay_stride, make_uint2(e.x, e.y), lc, A);
                 eval_quad<real, MODE>(s_base, pay_stride, make_uint2(e.z, e.w), lc, A);
-                if ((tg & 3) == 3) A.flush(dx, dy, dz);      // every 32 entries: FP32 partial -> FP64
+                if ((m_use & 3) == 0) A.flush(dx, dy, dz);   // every 32 entries: FP32 partial -> FP64
             }
         } else {
             // Two quads per trip; a quad is loaded one whole trip (8 pairs) before its use, right after
             // the registers it goes to have been unpacked.  The loads are volatile asm so that they
             // stay where they are written: a load that drifts to the end of the loop body shares its
             // scoreboard with the unpack at the top and exposes the full L2 latency in every trip.
-            const uint2 *pq = lp + qidx(q0);
-            const uint2 *const pend = lp + qidx(q1 - 2);           // clamp for the look-ahead loads
+            const int r0 = q0 >> 1;
+            const int qf = (r0 + ((part - r0) & (wpb - 1))) << 1;  // first quad of my first row in this chunk
+            if (qf >= q1) continue;
+            const int qstep = 2 * wpb;
+            const uint2 *pq = lp + qidx(qf);
+            const uint2 *const pend = lp + qidx(qf + ((q1 - 2 - qf) / qstep) * qstep);   // my last row: clamp for the look-ahead loads
+            const size_t pstep = (size_t)64 * wpb;
             uint2 eA = ldg_list(pq);
             uint2 eB = ldg_list(pq + 1);
-            for (int q = q0; q < q1; q += 2, pq += 64) {
+            for (int q = qf; q < q1; q += qstep, pq += pstep) {
                 const uint2 a = eA;
-                eA = ldg_list(pq + 64 <= pend ? pq + 64 : pend);
+                eA = ldg_list(pq + pstep <= pend ? pq + pstep : pend);
                 eval_quad<real, MODE>(s_base, pay_stride, a, lc, A);
                 const uint2 b = eB;
-                eB = ldg_list(pq + 64 <= pend ? pq + 65 : pend + 1);
+                eB = ldg_list(pq + pstep <= pend ? pq + pstep + 1 : pend + 1);
                 eval_quad<real, MODE>(s_base, pay_stride, b, lc, A);
                 if (++since_flush == 4) {          // every 32 entries: FP32 partial -> FP64 accumulator
                     A.flush(dx, dy, dz);
@@ -585,14 +599,27 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     }
     if (RING > 0) cp_async_wait<0>();
     A.flush(dx, dy, dz);
-    if (active) {
+    if (wpb > 1) {                             // uniform over the CTA: add the parts of a block, part 1 first
+        double *s_part = reinterpret_cast<double *>(smem_raw);         // [warp][xyz][lane], over the dead records
+        __syncthreads();
+        if (part > 0) {
+            s_part[w * 96 + lane] = dx; s_part[w * 96 + 32 + lane] = dy; s_part[w * 96 + 64 + lane] = dz;
+        }
+        __syncthreads();
+        if (part == 0)
+            for (int k = 1; k < wpb; ++k) {
+                dx += s_part[(w + k) * 96 + lane]; dy += s_part[(w + k) * 96 + 32 + lane]; dz += s_part[(w + k) * 96 + 64 + lane];
+            }
+    }
+    const bool owner = active && part == 0;
+    if (owner) {
         acc[slot] = dx;
         acc[n_pad + slot] = dy;
         acc[2 * (size_t)n_pad + slot] = dz;
     }
     if (MODE == MODE_TMU && fuse.on) {
         double pq = 0, dummy = 0;
-        if (active) {
+        if (owner) {
             const double ia = fuse.inv_alpha[slot];
             const double d[3] = {dx, dy, dz};
 #pragma unroll
