@@ -261,7 +261,7 @@ struct TmuLane {
     f2 pxy, nz0, one_w;
 };
 struct TmuConsts {
-    float pb;       // 0.4 beta:              u = 1 / (1 + pb R)
+    float pb;       // P beta (TKHP_ERFCX_P): u = 1 / (1 + pb R)
     float nb2l;     // -beta^2 log2 e:        e^{-z^2} = ex2(nb2l R^2)
     float c1b;      // (2/sqrt pi) beta:      c z
     float k3;       // (4/(3 sqrt pi)) beta^3: (2c/3) z^3 = k3 R^3

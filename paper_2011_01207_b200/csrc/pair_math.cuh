@@ -12,7 +12,7 @@
 // then scaled by R^-(2k+1):  R^3 bn1 = e^{-z^2}[erfcx(z) + c z],  R^5 bn2 = e^{-z^2}[3(..) + 2c z^3],
 // R^7 bn3 = e^{-z^2}[15(..) + 10 c z^3 + 4 c z^5],  z = bR, c = 2/sqrt(pi).
 //
-// MIXED (float): erfcx by the degree-8 polynomial of erfcx_coeffs.h in u = 1/(1+0.4z)
+// MIXED (float): erfcx by the degree-7 polynomial of erfcx_coeffs.h in u = 1/(1+0.35z)
 // (MUFU.RCP), exponentials by ex2.approx, 1/R by MUFU.RSQ: 4 MUFU + ~45 FMA-pipe ops per pair.
 // FP64 (double): erfc()/exp() of the CUDA math library.
 #pragma once
@@ -32,7 +32,7 @@ struct PairConsts {
     real box;       // box edge (PPI kernels)
     real inv_box;
     // products formed once on the host for the packed FP32 kernels (atom_pairs.cu)
-    real pb;        // 0.4 beta:                u = 1 / (1 + pb R)
+    real pb;        // P beta (P = TKHP_ERFCX_P): u = 1 / (1 + pb R)
     real nb2l;      // -beta^2 log2 e:          e^{-z^2} = ex2(nb2l R^2)
     real c1b;       // (2/sqrt pi) beta:        c z = c1b R
     real k3;        // (4/(3 sqrt pi)) beta^3:  (2c/3) z^3 = k3 R^3
