@@ -38,6 +38,11 @@ METRIC = "useful pair interactions/s (field + T.mu matvecs of one list-build + f
 UNIT = "pair interactions/s"
 FLOPS_PER_PAIR_TMU = 89      # 32 FFMA*2 + 22 FMUL + 3 FADD per evaluated slot
 FLOPS_PER_PAIR_FIELD = 160
+# What the ATOM-list MIXED T.mu kernel EXECUTES per evaluated slot (ordered pair), counted in the SASS
+# of its inner loop (8 slots per trip: 76 FFMA2 + 40 FMUL2 + 8 FADD2 + 51 FFMA + 24 FMUL, DESIGN.md
+# section 5.3): FMA-pipe lane-cycles (a packed instruction holds the pipe 2 cycles) and FP32 flops.
+TMU_ATOM_MIXED_PIPE_CYCLES_PER_SLOT = (2 * (76 + 40 + 8) + 51 + 24) / 8
+TMU_ATOM_MIXED_FLOPS_PER_SLOT = (4 * 76 + 2 * 40 + 2 * 8 + 2 * 51 + 24) / 8
 # ALU roofline denominator derived in DESIGN.md section 7: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 PEAK_FP64_TFLOPS = PEAK_FP32_TFLOPS / 2
@@ -273,8 +278,13 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "executed_frac_of_peak": executed / peak,
         "useful_pairs_per_s_kernel": n_pair / (tmu_ms * 1e-3),
         "field_kernel_avg_ms": fld_ms,
-        "peak_note": "148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md section 7)",
+        "peak_note": "148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
     }
+    if mode_in_use == pk.TKHP_LIST_ATOM and args.precision == "mixed":
+        lanes_per_s = 148 * 128 * 1.965e9
+        roofline["executed_flops_per_slot_sass"] = TMU_ATOM_MIXED_FLOPS_PER_SLOT
+        roofline["executed_tflops_sass"] = TMU_ATOM_MIXED_FLOPS_PER_SLOT * n_slots / (tmu_ms * 1e-3) / 1e12
+        roofline["fma_pipe_busy_frac"] = TMU_ATOM_MIXED_PIPE_CYCLES_PER_SLOT * n_slots / (tmu_ms * 1e-3) / lanes_per_s
     try:
         traffic_file = ROOT / "profiles" / "traffic.json"
         if traffic_file.exists():
@@ -321,7 +331,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
         oracle.build()
-        rows = 8192 if n > 20000 else n
+        rows = min(n, 131072)        # config 2: every row once, about 7 s on 16 cores
         r = oracle_sample(sys_, rows)
         cpu = {"value": r["pair_interactions"] / r["seconds"], "unit": UNIT, "cores": r["cores"],
                "kind": "oracle", "seconds": r["seconds"],
