@@ -52,7 +52,7 @@ WORKLOADS = {0: "cfg0_water648", 1: "cfg1_dhfr_size_23559", 2: "cfg2_hetero_9830
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3])
