@@ -104,17 +104,28 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             const uint4 cur = nxt;
             if (v + 1 < L8) nxt = ent8[v + 1];           // one address per quarter warp, one load ahead
             const unsigned word[4] = {cur.x, cur.y, cur.z, cur.w};
+            // the 8 entries of the vector are tested together (8 independent chains: the loop was bound
+            // by fixed-latency dependencies), then the hits are appended in list order
+            unsigned loc[8];
+            bool hit[8];
 #pragma unroll
             for (int h = 0; h < 8; ++h) {
                 const unsigned e = (word[h >> 1] >> ((h & 1) * 16)) & 0xffffu;
-                if ((int)e >= count) { open = false; break; }      // padding entries (== count) close the list
-                const unsigned loc = (e * magic) >> 20;            // e / n_chunks
-                if (e - loc * (unsigned)n_chunks != (unsigned)c) continue;
-                const vec4 pj = s_pos[loc];
+                loc[h] = (e * magic) >> 20;                        // e / n_chunks
+                hit[h] = (int)e < count && e - loc[h] * (unsigned)n_chunks == (unsigned)c;   // padding entries are == count
+                if (h == 7) open = (int)e < count;                 // padding only at the end of a list
+            }
+#pragma unroll
+            for (int h = 0; h < 8; ++h) {
+                const vec4 pj = s_pos[hit[h] ? loc[h] : 0u];
                 const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
                 const real r2 = Rx * Rx + Ry * Ry + Rz * Rz;
-                if (r2 <= rc2 && r2 > (real)1e-10) {
-                    pend |= (unsigned long long)(loc * (unsigned)sizeof(vec4)) << ((k & 3) * 16);
+                hit[h] = hit[h] && r2 <= rc2 && r2 > (real)1e-10;
+            }
+#pragma unroll
+            for (int h = 0; h < 8; ++h) {
+                if (hit[h]) {
+                    pend |= (unsigned long long)(loc[h] * (unsigned)sizeof(vec4)) << ((k & 3) * 16);
                     if ((k & 3) == 3) {
                         const int q = q0 + (k >> 2);
                         if (q < q_cap) out[qidx(q)] = make_uint2((unsigned)pend, (unsigned)(pend >> 32));
@@ -178,15 +189,20 @@ k_atom_reorder(ClusterWs ws, int n_blocks, int rec_bytes, int s_chunk) {
         const int len = (q1 - q0) << 2;                    // common padded length of this chunk's lists
         if (len <= 0) continue;
         if (len > RO_ROWS) continue;                       // image too small: keep staging order
-        for (int r = 0; r < RO_ROWS; ++r) img[r * 32] = 0xffffu;
-        // deal the entries into the per-bank columns
+        for (int r = 0; r < len; ++r) img[r * 32] = 0xffffu;     // rows >= len are only read where written
+        // deal the entries into the per-bank columns; a list row (8 entries = 16 B per lane) is
+        // loaded one row ahead of its use
         unsigned long long cnt = 0;                        // 8 counters of 8 bits
         bool fits = true;
-        for (int q = q0; q < q1; ++q) {
-            const uint2 e = list[qidx(q)];
-            const unsigned v[4] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16};
+        const uint4 *rowp = reinterpret_cast<const uint4 *>(list + qidx(q0));      // q0 is even: row q0 / 2
+        uint4 nxt = rowp[0];
+        for (int q = q0; q < q1; q += 2, rowp += 32) {
+            const uint4 e = nxt;
+            if (q + 2 < q1) nxt = rowp[32];
+            const unsigned v[8] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16,
+                                   e.z & 0xffffu, e.z >> 16, e.w & 0xffffu, e.w >> 16};
 #pragma unroll
-            for (int h = 0; h < 4; ++h) {
+            for (int h = 0; h < 8; ++h) {
                 if (v[h] == dummy) continue;
                 const unsigned b = (v[h] >> 4) & 7u;
                 const unsigned r = (unsigned)(cnt >> (8 * b)) & 0xffu;
@@ -210,14 +226,15 @@ k_atom_reorder(ClusterWs ws, int n_blocks, int rec_bytes, int s_chunk) {
             }
         }
         // write back; untouched holes (0xffff) are the padding
-        for (int q = q0; q < q1; ++q) {
-            unsigned v[4];
+        uint4 *outp = reinterpret_cast<uint4 *>(list + qidx(q0));
+        for (int q = q0; q < q1; q += 2, outp += 32) {
+            unsigned v[8];
 #pragma unroll
-            for (int h = 0; h < 4; ++h) {
+            for (int h = 0; h < 8; ++h) {
                 const unsigned x = img[(((q - q0) << 2) + h) * 32];
                 v[h] = x == 0xffffu ? dummy : x;
             }
-            list[qidx(q)] = make_uint2(v[0] | (v[1] << 16), v[2] | (v[3] << 16));
+            *outp = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
         }
         __syncwarp();
     }
