@@ -98,3 +98,31 @@ def test_cfg2_sampled_rows_mixed(cfg2, list_mode):
     e_g = float(P.polar_energy(mu_g, Eg).cpu())
     assert abs(e_g - oracle.polar_energy(mu_h, Eg.cpu().numpy())) <= 1e-12 * abs(e_g)
     P.close()
+
+
+@pytest.mark.parametrize("precision", ["mixed", "fp64"])
+def test_groups_of_3_and_4_blocks_split_between_two_warps(precision):
+    """A 48,000-atom box has 1,500 blocks in 444 groups of 3 or 4 blocks: every block is walked by two
+    warps (even and odd list rows) whose parts are added in a fixed order.  Sampled
+    rows against the oracle, the exact pair count, and bit-identical repeats."""
+    import paper_2011_01207_b200 as pk
+    from synth_inputs.generator import water_box
+    s = water_box(16000, 78.3, 4801, solute_frac=0.1)
+    P = pk.Polarizer.for_system(s, precision=pk.TKHP_FP64 if precision == "fp64" else pk.TKHP_MIXED,
+                                list_mode=pk.TKHP_LIST_ATOM)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    n_pair, n_slots, mode = P.nblist_stats()
+    assert mode == pk.TKHP_LIST_ATOM and n_pair == oracle.count_pairs(s)
+    perm, _ = P.nblist_view()
+    n_blocks = perm.size // 32
+    assert 3 <= n_blocks / 444 <= 4
+    rows = _rows(s, perm, n_rand=768, n_blocks=6, seed=3)
+    tol = 1e-11 if precision == "fp64" else 1e-5
+    rng = np.random.default_rng(4)
+    mu = rng.standard_normal((s.n_atoms, 3)) * 0.1
+    a = P.tmatvec(mu).cpu().numpy()
+    assert _rel_l2(a[rows], oracle.tmatvec_rows(s, mu, rows)) <= tol
+    assert np.array_equal(a, P.tmatvec(mu).cpu().numpy())
+    Eg = P.perm_field(s.charge, s.dipole, s.quad).cpu().numpy()
+    assert _rel_l2(Eg[rows], oracle.perm_field_rows(s, rows)) <= tol
+    P.close()
