@@ -171,7 +171,8 @@ int tkhp_polar_energy(tkhp_ctx *ctx, const double *d_mu, const double *d_field,
  * Whole hot path from HOST buffers (end-to-end entry used for the e2e benchmark leg):
  * copies the inputs to the device, builds the list, evaluates the field, solves for mu,
  * computes E_pol and copies mu, field and E_pol back.  Host arrays as in the calls above.
- * The staging buffers come from the context's workspace.  Synchronises.
+ * The staging buffers come from the context's workspace; the multipole copies run on a stream of
+ * the context beside the list build.  Synchronises.
  */
 int tkhp_polarize_host(tkhp_ctx *ctx, const double *h_pos, const double *h_polarizability,
                        const int32_t *h_group_id, const double *h_charge, const double *h_dipole,

@@ -208,6 +208,8 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
         return TKHP_ECUDA;
     }
     for (int i = 0; i < 10; ++i) cudaEventCreate(&c->ev[i]);
+    cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; i < 2; ++i) cudaEventCreateWithFlags(&c->copy_ev[i], cudaEventDisableTiming);
     for (int w = 0; w < 2; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventCreate(&c->prof_ev[w][i]);
     for (int i = 0; i < 5; ++i) c->last_ms[i] = -1.0;
@@ -225,6 +227,8 @@ int tkhp_destroy(tkhp_ctx *ctx) {
     cudaSetDevice(c->p.device);
     cudaDeviceSynchronize();
     for (int i = 0; i < 10; ++i) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < 2; ++i) cudaEventDestroy(c->copy_ev[i]);
+    cudaStreamDestroy(c->copy_stream);
     for (int w = 0; w < 2; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventDestroy(c->prof_ev[w][i]);
     cudaFreeHost(c->h_ring);
@@ -370,13 +374,19 @@ int tkhp_polarize_host(tkhp_ctx *ctx, const double *h_pos, const double *h_polar
     TKHP_CUDA(c, cudaMemcpyAsync(c->h_pos, h_pos, 24 * n, cudaMemcpyHostToDevice, s));
     TKHP_CUDA(c, cudaMemcpyAsync(c->h_alpha, h_polarizability, 8 * n, cudaMemcpyHostToDevice, s));
     TKHP_CUDA(c, cudaMemcpyAsync(c->h_group, h_group_id, 4 * n, cudaMemcpyHostToDevice, s));
-    TKHP_CUDA(c, cudaMemcpyAsync(c->h_charge, h_charge, 8 * n, cudaMemcpyHostToDevice, s));
-    TKHP_CUDA(c, cudaMemcpyAsync(c->h_dipole, h_dipole, 24 * n, cudaMemcpyHostToDevice, s));
-    TKHP_CUDA(c, cudaMemcpyAsync(c->h_quad, h_quad, 48 * n, cudaMemcpyHostToDevice, s));
+    // the multipoles (80 of the 116 bytes per atom) are not needed before the field: their copies
+    // run on a second stream beside the list build (copy engine and SMs at the same time)
+    TKHP_CUDA(c, cudaEventRecord(c->copy_ev[0], s));               // after whatever the caller queued on s
+    TKHP_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->copy_ev[0], 0));
+    TKHP_CUDA(c, cudaMemcpyAsync(c->h_charge, h_charge, 8 * n, cudaMemcpyHostToDevice, c->copy_stream));
+    TKHP_CUDA(c, cudaMemcpyAsync(c->h_dipole, h_dipole, 24 * n, cudaMemcpyHostToDevice, c->copy_stream));
+    TKHP_CUDA(c, cudaMemcpyAsync(c->h_quad, h_quad, 48 * n, cudaMemcpyHostToDevice, c->copy_stream));
+    TKHP_CUDA(c, cudaEventRecord(c->copy_ev[1], c->copy_stream));
     int rc = tkhp_nblist_build(ctx, c->h_pos, c->h_alpha, c->h_group, stream);
-    if (rc) return rc;
+    if (rc) { cudaStreamSynchronize(c->copy_stream); return rc; }
+    TKHP_CUDA(c, cudaStreamWaitEvent(s, c->copy_ev[1], 0));
     rc = tkhp_perm_field(ctx, c->h_charge, c->h_dipole, c->h_quad, c->h_field, stream);
-    if (rc) return rc;
+    if (rc) { cudaStreamSynchronize(c->copy_stream); return rc; }     // the caller may free its buffers
     int rc_solve = tkhp_polar_solve(ctx, c->h_field, c->h_mu, tol, max_iter, 0, h_iters, h_rms, stream);
     if (rc_solve && rc_solve != TKHP_ENOCONV) return rc_solve;
     rc = tkhp_polar_energy(ctx, c->h_mu, c->h_field, c->h_energy, stream);

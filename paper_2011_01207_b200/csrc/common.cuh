@@ -111,6 +111,8 @@ struct Ctx {
     bool header_valid;
     // host-entry staging (tkhp_polarize_host)
     double *h_pos, *h_alpha, *h_charge, *h_dipole, *h_quad, *h_field, *h_mu, *h_energy;
+    cudaStream_t copy_stream;   // tkhp_polarize_host: the multipole H2D copies run beside the list build
+    cudaEvent_t copy_ev[2];
     int32_t *h_group;
     // CLUSTER mode lists (see cluster.cu)
     void *cl_ws;
