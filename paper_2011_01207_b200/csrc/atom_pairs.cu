@@ -19,7 +19,9 @@
 //    cp.async, several trips ahead (the L2/HBM latency of this stream was the largest stall of
 //    the register-prefetch version); the other variants load them one trip ahead into registers;
 //  * the loss of coalescing the paper notes becomes per-lane LDS.128 gathers from shared memory;
-//    two pairs are evaluated together per lane (two independent dependency chains);
+//    two pairs are evaluated together per lane: in the FP32 T.mu kernel as the two halves of
+//    packed FP32 instructions (f32x2.cuh), elsewhere as two independent dependency chains;
+//  * a group with fewer than 5 blocks gives every block to 2, 4 or 8 warps (interleaved list rows);
 //  * FP32 partial sums are flushed into FP64 registers every 32 entries.
 // The lists are built from the CLUSTER lists (the 8-atom-cluster list is the candidate set of
 // each of its atoms): k_atom_lists below.
@@ -381,12 +383,6 @@ __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_
     }
 }
 
-// pairs evaluated together per lane (independent dependency chains): 4 in the FP32 T.mu kernel
-// (a 98k-atom system has only ~21 warps per SM, so the latency must be covered inside the warp),
-// 2 elsewhere (register budget)
-template <typename real, int MODE> struct PairWidth { static constexpr int W = 2; };
-template <> struct PairWidth<float, MODE_TMU> { static constexpr int W = 2; };   // 4 measured slower (80 registers)
-
 // one lane's quad of list entries (8 bytes), read-only path, pinned in program order
 __device__ __forceinline__ uint2 ldg_list(const uint2 *p) {
     uint2 v;
@@ -410,14 +406,10 @@ struct LaneCtx<float, MODE_TMU> {
 template <typename real, int MODE>
 __device__ __forceinline__ void eval_quad(const unsigned char *s_base, int pay_stride, uint2 e,
                                           const LaneCtx<real, MODE> &lc, Partial<real, MODE> &A) {
-    if (PairWidth<real, MODE>::W == 4) {
-        const unsigned off[4] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16};
-        eval_pairs<real, MODE, 4>(s_base, pay_stride, off, lc.pi, lc.gi, lc.kc, A);
-    } else {
-        const unsigned o0[2] = {e.x & 0xffffu, e.x >> 16}, o1[2] = {e.y & 0xffffu, e.y >> 16};
-        eval_pairs<real, MODE, 2>(s_base, pay_stride, o0, lc.pi, lc.gi, lc.kc, A);
-        eval_pairs<real, MODE, 2>(s_base, pay_stride, o1, lc.pi, lc.gi, lc.kc, A);
-    }
+    // two pairs at a time (two independent dependency chains; four measured slower: registers)
+    const unsigned o0[2] = {e.x & 0xffffu, e.x >> 16}, o1[2] = {e.y & 0xffffu, e.y >> 16};
+    eval_pairs<real, MODE, 2>(s_base, pay_stride, o0, lc.pi, lc.gi, lc.kc, A);
+    eval_pairs<real, MODE, 2>(s_base, pay_stride, o1, lc.pi, lc.gi, lc.kc, A);
 }
 template <>
 __device__ __forceinline__ void eval_quad<float, MODE_TMU>(const unsigned char *s_base, int pay_stride, uint2 e,
