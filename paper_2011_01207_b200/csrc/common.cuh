@@ -49,7 +49,7 @@ struct DeviceState {
     double rzv[2];          // r.z ping-pong (iteration parity)
     double pq, rr, gamma, delta;
     unsigned ticket;        // last-block reductions (reduce.cuh); 0 between kernels
-    int pad2;
+    int bar_gen;            // grid barrier of k_pcg_step: the iteration whose partial sums are complete
     int conv_at;            // PCG: iterations with index >= conv_at are skipped on the device
     int iters;
 };

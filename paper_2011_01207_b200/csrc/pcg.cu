@@ -124,7 +124,7 @@ __global__ void k_pcg_init(const double *__restrict__ field, const double *__res
                            double *__restrict__ vE, double *__restrict__ vmu, vec4 *__restrict__ packed,
                            DeviceState *st) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s == 0) { st->conv_at = 0x7fffffff; st->iters = 0; st->ticket = 0u; }
+    if (s == 0) { st->conv_at = 0x7fffffff; st->iters = 0; st->ticket = 0u; st->bar_gen = -1; }
     if (s >= n_pad) return;
     const int a = perm[s];
     double e[3] = {0, 0, 0}, m[3] = {0, 0, 0};
@@ -225,6 +225,73 @@ __global__ void k_pcg_direction(const double *__restrict__ vr, const double *__r
         }
         store_vec(packed, s, p[0], p[1], p[2]);
     }
+}
+
+// One PCG iteration's vector work in ONE cooperative launch (all blocks resident): the update
+// (gamma = rz/pq; mu += gamma p; r -= gamma q; partial r.z, r.r), a grid barrier, then the direction
+// (delta = rz_new/rz_old; p = alpha r + delta p; pack p) from the r, alpha and p still in registers.
+// Every block adds the partial sums of all blocks in the same order, so all of them hold identical
+// totals and take the same convergence decision; block 0 publishes.  Replaces k_pcg_update +
+// k_pcg_direction: one launch and one pass over r, alpha, p less per iteration.  One atom per thread.
+template <typename vec4>
+__global__ void __launch_bounds__(RED_THREADS)
+k_pcg_step(double *__restrict__ vp, const double *__restrict__ vq, const double *__restrict__ alpha_s, int n_pad,
+           double *__restrict__ vmu, double *__restrict__ vr, vec4 *__restrict__ packed, double *__restrict__ part,
+           DeviceState *st, int iter, double tol, int n_atoms, volatile double *ring_slot) {
+    if (iter >= st->conv_at) return;
+    const double rz_old = st->rzv[iter & 1];
+    const double gamma = rz_old / st->pq;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    double al = 0.0, r[3] = {0, 0, 0}, p[3] = {0, 0, 0};
+    double rz = 0, rr = 0;
+    if (s < n_pad) {
+        al = alpha_s[s];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const size_t o = (size_t)c * n_pad + s;
+            p[c] = vp[o];
+            vmu[o] += gamma * p[c];
+            r[c] = vr[o] - gamma * vq[o];
+            vr[o] = r[c];
+            rz += r[c] * (al * r[c]); rr += r[c] * r[c];
+        }
+    }
+    block_sum2(rz, rr);
+    // ---- grid barrier: partials out, last arriver opens the gate for this iteration
+    __shared__ double s_tot[2];
+    if (threadIdx.x == 0) {
+        part[2 * blockIdx.x] = rz;
+        part[2 * blockIdx.x + 1] = rr;
+        __threadfence();
+        if (atomicInc(&st->ticket, gridDim.x - 1) == gridDim.x - 1) {
+            __threadfence();
+            *reinterpret_cast<volatile int *>(&st->bar_gen) = iter;
+        } else {
+            while (*reinterpret_cast<volatile int *>(&st->bar_gen) != iter) {}
+        }
+        __threadfence();
+    }
+    __syncthreads();
+    double x = 0, y = 0;
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += RED_THREADS) {
+        x += __ldcg(part + 2 * i);
+        y += __ldcg(part + 2 * i + 1);
+    }
+    block_sum2(x, y);
+    if (threadIdx.x == 0) { s_tot[0] = x; s_tot[1] = y; }
+    __syncthreads();
+    const double rz_new = s_tot[0], rr_new = s_tot[1];
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        pcg_publish_residual(st, (iter + 1) & 1, rz_new, rr_new, iter + 1, tol, n_atoms, ring_slot);
+    if (sqrt(rr_new / n_atoms) < tol) return;          // converged: no new direction (same test as the host's)
+    if (s >= n_pad) return;
+    const double delta = rz_new / rz_old;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        p[c] = al * r[c] + delta * p[c];
+        vp[(size_t)c * n_pad + s] = p[c];
+    }
+    store_vec(packed, s, p[0], p[1], p[2]);
 }
 
 __global__ void k_unsort3(const double *__restrict__ v, const int32_t *__restrict__ perm, int n_pad,
@@ -358,6 +425,16 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
     double *part_pq = c->partials + 2 * (size_t)c->part_cap;
     const bool fused_q = c->list_mode_in_use == TKHP_LIST_ATOM;   // q and p.q in the pair kernel's epilogue
     int rc;
+    // the fused update+direction kernel has a grid barrier: one atom per thread and every block resident
+    bool fused_step = false;
+    {
+        int per_sm = 0;
+        const void *fn = mixed ? (const void *)k_pcg_step<float4> : (const void *)k_pcg_step<double4>;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, VEC_THREADS, 0) == cudaSuccess)
+            fused_step = g1 <= per_sm * c->sm_count && g1 <= c->part_cap;
+        else
+            cudaGetLastError();
+    }
 
     for (int k = 0; k < RING; ++k) c->h_ring[k] = -1.0;
     const int prof_first = c->prof_n[0];
@@ -390,12 +467,24 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
                 k_pcg_q<<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vp, c->inv_alpha_s, self, n_pad, c->vq, part_pq, c->st, enq);
                 c->n_launches += 1;
             }
-            k_pcg_update<<<gv, VEC_THREADS, 0, s>>>(c->vp, c->vq, c->alpha_s, n_pad, c->vmu, c->vr, part_rz, c->st, enq, tol, c->n, c->d_ring + slot);
-            if (mixed)
-                k_pcg_direction<float4><<<gv, VEC_THREADS, 0, s>>>(c->vr, c->alpha_s, n_pad, c->vp, c->mu32, c->st, enq);
-            else
-                k_pcg_direction<double4><<<gv, VEC_THREADS, 0, s>>>(c->vr, c->alpha_s, n_pad, c->vp, c->mu64, c->st, enq);
-            c->n_launches += 2;   // update, direction
+            if (fused_step) {
+                // one cooperative launch: update, grid barrier, direction (k_pcg_step)
+                double *a_vp = c->vp; const double *a_vq = c->vq; const double *a_al = c->alpha_s; int a_n = n_pad;
+                double *a_mu = c->vmu; double *a_r = c->vr; void *a_pk = mixed ? (void *)c->mu32 : (void *)c->mu64;
+                double *a_part = part_rz; DeviceState *a_st = c->st; int a_it = enq; double a_tol = tol; int a_na = c->n;
+                volatile double *a_ring = c->d_ring + slot;
+                void *args[] = {&a_vp, &a_vq, &a_al, &a_n, &a_mu, &a_r, &a_pk, &a_part, &a_st, &a_it, &a_tol, &a_na, &a_ring};
+                const void *fn = mixed ? (const void *)k_pcg_step<float4> : (const void *)k_pcg_step<double4>;
+                TKHP_CUDA(c, cudaLaunchCooperativeKernel(fn, dim3(g1), dim3(VEC_THREADS), args, 0, s));
+                c->n_launches += 1;
+            } else {
+                k_pcg_update<<<gv, VEC_THREADS, 0, s>>>(c->vp, c->vq, c->alpha_s, n_pad, c->vmu, c->vr, part_rz, c->st, enq, tol, c->n, c->d_ring + slot);
+                if (mixed)
+                    k_pcg_direction<float4><<<gv, VEC_THREADS, 0, s>>>(c->vr, c->alpha_s, n_pad, c->vp, c->mu32, c->st, enq);
+                else
+                    k_pcg_direction<double4><<<gv, VEC_THREADS, 0, s>>>(c->vr, c->alpha_s, n_pad, c->vp, c->mu64, c->st, enq);
+                c->n_launches += 2;   // update, direction
+            }
             ++enq;
         }
         if ((rc = wait_slot(c, s, seen % RING, &rr))) return rc;
@@ -405,7 +494,8 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
     }
     // speculative iterations enqueued after convergence returned at once: keep them out of the counts
     if (rms < tol) {
-        c->n_noop_launches += (fused_q ? 3LL : 4LL) * (enq - it) + (it > 0 ? 1 : 0);   // + the last direction
+        if (fused_step) c->n_noop_launches += (fused_q ? 2LL : 3LL) * (enq - it);
+        else c->n_noop_launches += (fused_q ? 3LL : 4LL) * (enq - it) + (it > 0 ? 1 : 0);   // + the last direction
         for (int i = prof_first; i < c->prof_n[0]; ++i)
             if (c->prof_iter[0][i] >= it) c->prof_skip[0][i] = true;
     }
