@@ -281,17 +281,20 @@ k_pcg_step(double *__restrict__ vp, const double *__restrict__ vq, const double 
     if (threadIdx.x == 0) { s_tot[0] = x; s_tot[1] = y; }
     __syncthreads();
     const double rz_new = s_tot[0], rr_new = s_tot[1];
+    const bool converged = sqrt(rr_new / n_atoms) < tol;      // same test as the host's: no new direction then
+    if (!converged && s < n_pad) {
+        const double delta = rz_new / rz_old;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            p[c] = al * r[c] + delta * p[c];
+            vp[(size_t)c * n_pad + s] = p[c];
+        }
+        store_vec(packed, s, p[0], p[1], p[2]);
+    }
+    // the scalars and the host's copy of |r|^2 last: the system-scope fence of the publish is off the
+    // other blocks' path and behind block 0's own stores
     if (blockIdx.x == 0 && threadIdx.x == 0)
         pcg_publish_residual(st, (iter + 1) & 1, rz_new, rr_new, iter + 1, tol, n_atoms, ring_slot);
-    if (sqrt(rr_new / n_atoms) < tol) return;          // converged: no new direction (same test as the host's)
-    if (s >= n_pad) return;
-    const double delta = rz_new / rz_old;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        p[c] = al * r[c] + delta * p[c];
-        vp[(size_t)c * n_pad + s] = p[c];
-    }
-    store_vec(packed, s, p[0], p[1], p[2]);
 }
 
 __global__ void k_unsort3(const double *__restrict__ v, const int32_t *__restrict__ perm, int n_pad,
