@@ -134,6 +134,14 @@ int tkhp_nblist_view(tkhp_ctx *ctx, int32_t *n_blocks, int64_t *n_pairs,
 int tkhp_nblist_stats(tkhp_ctx *ctx, int64_t *n_pairs_within_cutoff, int64_t *n_slots_evaluated,
                       int32_t *list_mode_in_use, void *stream);
 
+/* Break-down of the ATOM lists ("list filtering", carried down to the atom; DESIGN.md
+ * section 5.3).  Synchronises `stream`.  out[0] = lane-slots in FAR rows (pairs evaluated without
+ * the Thole term), out[1] = lane-slots in NEAR rows (full formula), out[2] = list segments summed
+ * over blocks, out[3] = 1 if the far class is in use (MIXED precision and ewald_beta > 0), else 0
+ * (then every slot is counted in out[0] and evaluated with the full formula).  All zero unless
+ * the list mode in use is TKHP_LIST_ATOM.  TKHP_ENOLIST before a build.                      */
+int tkhp_nblist_atom_stats(tkhp_ctx *ctx, int64_t out[4], void *stream);
+
 /*
  * Permanent-multipole field (F1-F3; charge, dipole, traceless quadrupole,
  * erfc-damped real-space Ewald with Thole damping; same-group pairs masked; Ewald self

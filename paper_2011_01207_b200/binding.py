@@ -17,7 +17,7 @@ _ERR_NAMES = {-1: "TKHP_EINVAL", -2: "TKHP_ECUDA", -3: "TKHP_ECUTOFF", -4: "TKHP
 
 EXPORTED_SYMBOLS = [
     "tkhp_workspace_bytes", "tkhp_create", "tkhp_destroy", "tkhp_last_error",
-    "tkhp_nblist_build", "tkhp_nblist_view", "tkhp_nblist_stats", "tkhp_perm_field",
+    "tkhp_nblist_build", "tkhp_nblist_view", "tkhp_nblist_stats", "tkhp_nblist_atom_stats", "tkhp_perm_field",
     "tkhp_tmatvec", "tkhp_polar_solve", "tkhp_polar_energy", "tkhp_polarize_host",
     "tkhp_last_timings", "tkhp_fma_peak", "tkhp_profile_reset", "tkhp_profile_read",
 ]
@@ -66,6 +66,7 @@ def lib() -> ctypes.CDLL:
                                        POINTER(c_void_p), POINTER(c_void_p), vp]
         L.tkhp_nblist_stats.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64),
                                         POINTER(c_int32), vp]
+        L.tkhp_nblist_atom_stats.argtypes = [c_void_p, POINTER(c_int64), vp]
         L.tkhp_perm_field.argtypes = [c_void_p, dp, dp, dp, dp, vp]
         L.tkhp_tmatvec.argtypes = [c_void_p, dp, dp, vp]
         L.tkhp_polar_solve.argtypes = [c_void_p, dp, dp, c_double, c_int32, c_int32,
@@ -152,6 +153,13 @@ def tkhp_nblist_stats(ctx, stream=None, count_pairs: bool = True):
     _check(lib().tkhp_nblist_stats(ctx, byref(npair) if count_pairs else None, byref(nslot),
                                    byref(mode), _stream_ptr(stream)), ctx)
     return (npair.value if count_pairs else None), nslot.value, mode.value
+
+
+def tkhp_nblist_atom_stats(ctx, stream=None):
+    """-> (far lane-slots, near lane-slots, segments, far class in use) of the ATOM lists."""
+    out = (c_int64 * 4)()
+    _check(lib().tkhp_nblist_atom_stats(ctx, out, _stream_ptr(stream)), ctx)
+    return int(out[0]), int(out[1]), int(out[2]), bool(out[3])
 
 
 def tkhp_perm_field(ctx, d_charge, d_dipole, d_quad, d_field, stream=None):
@@ -295,6 +303,9 @@ class Polarizer:
 
     def nblist_stats(self, stream=None, count_pairs=True):
         return tkhp_nblist_stats(self.ctx, stream, count_pairs)
+
+    def nblist_atom_stats(self, stream=None):
+        return tkhp_nblist_atom_stats(self.ctx, stream)
 
     def perm_field(self, charge, dipole, quad, out=None, stream=None):
         q, d, th = self._f64(charge), self._f64(dipole), self._f64(quad)

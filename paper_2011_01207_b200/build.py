@@ -17,7 +17,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 OBJ = PKG / "build"
 LIB = PKG / "libtkhp.so"
-SOURCES = ["api.cu", "nblist.cu", "tiles.cu", "cluster_build.cu", "cluster_pairs.cu", "atom_pairs.cu", "pcg.cu", "fma_peak.cu"]
+SOURCES = ["api.cu", "nblist.cu", "tiles.cu", "cluster_build.cu", "cluster_pairs.cu", "atom_lists.cu", "atom_pairs.cu", "pcg.cu", "fma_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false"]
 
@@ -40,7 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     headers = list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.h")) + [PKG.parent / "include" / "tkhp.h"]
     nvcc = _nvcc()
-    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
+    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"] + os.environ.get("TKHP_NVCC_EXTRA", "").split()
 
     def compile_one(src: str):
         obj = OBJ / (src + ".o")

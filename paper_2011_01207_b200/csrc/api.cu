@@ -195,6 +195,12 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, params->device) != cudaSuccess) { delete c; return TKHP_ECUDA; }
     c->sm_count = prop.multiProcessorCount;
+    atom_far_setup(c);
+    if (cluster_pairs_configure(c) || atom_lists_configure(c) || atom_pairs_configure(c)) {
+        snprintf(g_create_err, sizeof(g_create_err), "%s", c->err);
+        delete c;
+        return TKHP_ECUDA;
+    }
     c->spec_iter = -1;
     c->fuse_q = false;
     c->n_noop_launches = 0;
@@ -306,6 +312,21 @@ int tkhp_nblist_stats(tkhp_ctx *ctx, int64_t *n_pairs_within_cutoff, int64_t *n_
         }
     }
     if (list_mode_in_use) *list_mode_in_use = c->list_mode_in_use;
+    return TKHP_OK;
+}
+
+int tkhp_nblist_atom_stats(tkhp_ctx *ctx, int64_t out[4], void *stream) {
+    if (!ctx || !out) return TKHP_EINVAL;
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    int rc = ensure_header(c, static_cast<cudaStream_t>(stream));
+    if (rc) return rc;
+    out[0] = out[1] = out[2] = out[3] = 0;
+    if (c->list_mode_in_use != TKHP_LIST_ATOM) return TKHP_OK;
+    const DeviceState &h = *c->h_state;
+    out[0] = 32LL * h.n_atom_far;
+    out[1] = 32LL * (h.n_atom_entries - h.n_atom_far);
+    out[2] = h.n_atom_segments;
+    out[3] = c->far_on ? 1 : 0;
     return TKHP_OK;
 }
 

@@ -37,6 +37,8 @@ constexpr int RESIDENT = 3;           // CTAs per SM the group count is rounded 
 constexpr int B200_SMS = 148;
 constexpr float GUARD = 0.01f;        // list radius = r_c + GUARD (FP32 build arithmetic is safe)
 constexpr int NCH_MAX = 16;           // ATOM mode: max staging chunks per group
+constexpr int NSEG_MAX = 2 * NCH_MAX; // ATOM mode: list segments (descriptors) per block, incl. the terminator
+constexpr int NEAR_CAP = 48;          // ATOM mode builder: near entries per lane and segment (image rows)
 constexpr int ATOM_SMEM = 56 * 1024;  // ATOM mode: shared memory of the T.mu kernel per CTA (4 CTAs / SM)
 
 // ATOM mode chunking of a group's staged atoms.  The shared-memory chunk holds s_max records; a
@@ -52,6 +54,29 @@ __host__ __device__ inline int atom_chunks_of(int count, int s_chunk) {
     return count < 1 ? 1 : (count + s_chunk - 1) / s_chunk;
 }
 
+// Rows of the far image the list builder keeps per warp (atom_lists.cu): 1.25 x the expected number
+// of neighbours of an atom in one chunk + 24, so that a chunk normally needs one segment (an
+// under-estimate only costs padding: the builder starts another segment when the image is full).
+inline int atom_far_cap(const tkhp_params *p, int n_blocks, int n_groups, bool f64) {
+    double per_chunk = 96.0;
+    if (p->box > 0.0) {
+        const double rho = p->n_atoms / (p->box * p->box * p->box);
+        const double nb = 4.18879 * p->cutoff * p->cutoff * p->cutoff * rho;
+        // staged atoms of a typical group: its atoms fill a (somewhat elongated) cube, widened by r_c
+        const double atoms = (double)BLOCK * n_blocks / n_groups;
+        double edge = 1.25 * cbrt(atoms / rho) + 2.0 * p->cutoff;
+        if (edge > p->box) edge = p->box;
+        const double staged = 0.45 * rho * edge * edge * edge;     // a low estimate: fewer chunks, larger image
+        const int chunk = atom_chunk_capacity(f64, p->max_stage_per_chunk);
+        const int n_chunks = (int)(staged / chunk) + 1;
+        per_chunk = nb / n_chunks;
+    }
+    int cap = ((int)(1.25 * per_chunk) + 24 + 15) & ~15;
+    if (cap < 32) cap = 32;
+    if (cap > 224) cap = 224;           // 16 KB of image per warp
+    return cap;
+}
+
 struct ClusterWs {
     int n_groups, s_cap, l_cap;
     int32_t *group_first;             // n_groups + 1
@@ -64,14 +89,28 @@ struct ClusterWs {
     uint32_t *stage_mask;             // n_groups * s_cap: which clusters of the group list the atom
     uint16_t *entries;                // (n_pad/8) * l_cap
     int32_t *oct_len;                 // n_pad/8: padded list length (equal within a warp)
-    // ATOM list mode (atom_pairs.cu): per-atom lists, one u16 BYTE OFFSET into the staged chunk per
-    // entry, laid out per block as [entry/4][lane][entry%4] so that a lane reads 4 entries with one
-    // coalesced 8-byte load; every chunk's list is padded to the longest lane of the warp.
+    // ATOM list mode (atom_lists.cu, atom_pairs.cu): per-atom lists, one u16 BYTE OFFSET into the
+    // staged chunk per entry (record index * 16 in MIXED, * 32 in FP64), laid out per block as ROWS
+    // [row][lane][8 entries]: 16 bytes per lane, one coalesced 512-byte row per warp.  A block's
+    // rows are a sequence of SEGMENTS, each described by one int2 of `aseg`:
+    //   x = first row | chunk << 24,   y = far calls | near calls << 16   (a call = 2 entries)
+    // the FAR rows (pairs whose Thole damping has died out and whose z = beta R lies in the range
+    // of the far-field fit: no Thole term, 2 MUFU) come first, the NEAR rows follow on the next row
+    // boundary; both are padded to the longest lane of the warp in units of one call.  A chunk
+    // normally has one segment; the builder starts another when its shared-memory image is full.
+    // The sequence ends with a terminator (chunk 0xff, x & 0xffffff = total rows of the block), which
+    // is repeated in the last slot of the block's descriptors.
     int chunk_cap;                    // tkhp_params.max_stage_per_chunk (0 = automatic)
-    int a_cap;                        // entries per lane and block (multiple of 4)
+    int a_cap;                        // entries per lane and block (multiple of 8)
+    int far_cap;                      // builder image: far entries per lane and segment (multiple of 16)
     uint16_t *alist;                  // n_blocks * a_cap * 32
-    int32_t *arow;                    // n_blocks * (NCH_MAX + 1): first entry of each chunk's list
+    int2 *aseg;                       // n_blocks * NSEG_MAX
 };
+
+__host__ __device__ __forceinline__ int seg_chunk(int2 d) { return (int)((unsigned)d.x >> 24); }
+__host__ __device__ __forceinline__ int seg_row0(int2 d) { return d.x & 0xffffff; }
+__host__ __device__ __forceinline__ int seg_far_calls(int2 d) { return d.y & 0xffff; }
+__host__ __device__ __forceinline__ int seg_near_calls(int2 d) { return (int)((unsigned)d.y >> 16); }
 
 inline int choose_groups(int n_blocks) {
     const int base = (n_blocks + GB - 1) / GB;
@@ -123,7 +162,7 @@ inline size_t carve_cluster(const tkhp_params *p, int n_blocks, void *base, Clus
     ws.stage_mask = w.take<uint32_t>(gs);
     ws.entries = w.take<uint16_t>((n_pad / CLUSTER) * ws.l_cap);
     ws.oct_len = w.take<int32_t>(n_pad / CLUSTER);
-    ws.a_cap = 0; ws.alist = nullptr; ws.arow = nullptr;
+    ws.a_cap = 0; ws.far_cap = 0; ws.alist = nullptr; ws.aseg = nullptr;
     ws.chunk_cap = p->max_stage_per_chunk;
     if (p->list_mode == TKHP_LIST_ATOM) {
         long long a;
@@ -132,14 +171,15 @@ inline size_t carve_cluster(const tkhp_params *p, int n_blocks, void *base, Clus
         } else if (p->box > 0.0) {
             const double rho = p->n_atoms / (p->box * p->box * p->box);
             const double r = p->cutoff + 0.05;
-            a = (long long)(1.6 * 4.18879 * r * r * r * rho) + 48;
+            a = (long long)(1.6 * 4.18879 * r * r * r * rho) + 112;
         } else {
             a = 1024;
         }
-        if (a > (long long)n_pad + 8 * NCH_MAX) a = (long long)n_pad + 8 * NCH_MAX;
+        if (a > (long long)n_pad + 16 * NCH_MAX) a = (long long)n_pad + 16 * NCH_MAX;
         ws.a_cap = (int)((a + 7) & ~7LL);
+        ws.far_cap = atom_far_cap(p, n_blocks, ws.n_groups, f64);
         ws.alist = w.take<uint16_t>((size_t)n_blocks * ws.a_cap * 32);
-        ws.arow = w.take<int32_t>((size_t)n_blocks * (NCH_MAX + 1));
+        ws.aseg = w.take<int2>((size_t)n_blocks * NSEG_MAX);
     }
     w.take<char>(256);
     if (out) *out = ws;

@@ -162,13 +162,7 @@ static int launch_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     if (need < s_chunk) s_chunk = need;
     if (s_chunk < 32) s_chunk = 32;
     const size_t smem = per * (size_t)(s_chunk + 1);
-    static bool configured[2][2] = {{false, false}, {false, false}};
     const int which = sizeof(real) == 8;
-    if (!configured[which][MODE]) {
-        TKHP_CUDA(c, cudaFuncSetAttribute(k_cluster_pairs<real, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          SMEM_BUDGET + 1024));
-        configured[which][MODE] = true;
-    }
     PairConsts<real> k = {};
     k.beta = (real)c->p.ewald_beta;
     k.c1 = (real)(2.0 / SQRT_PI);
@@ -184,6 +178,15 @@ static int launch_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     k_cluster_pairs<real, MODE><<<ws.n_groups, GT, smem, s>>>(ws, gpos, spos, data, k, c->acc, c->n_pad, s_chunk, c->st, c->spec_iter);
     c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
+    return TKHP_OK;
+}
+
+// dynamic shared memory opt-in, once per context (the attribute is per device)
+int cluster_pairs_configure(Ctx *c) {
+    TKHP_CUDA(c, cudaFuncSetAttribute(k_cluster_pairs<float, MODE_TMU>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + 1024));
+    TKHP_CUDA(c, cudaFuncSetAttribute(k_cluster_pairs<float, MODE_FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + 1024));
+    TKHP_CUDA(c, cudaFuncSetAttribute(k_cluster_pairs<double, MODE_TMU>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + 1024));
+    TKHP_CUDA(c, cudaFuncSetAttribute(k_cluster_pairs<double, MODE_FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET + 1024));
     return TKHP_OK;
 }
 

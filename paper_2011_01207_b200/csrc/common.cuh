@@ -43,6 +43,8 @@ struct DeviceState {
     long long n_cluster_entries;        // total entries of all cluster lists (CLUSTER mode)
     long long n_pairs_within_cutoff;    // statistics (tkhp_nblist_stats)
     long long n_atom_entries;           // ATOM mode: padded per-lane list entries summed over blocks
+    long long n_atom_far;               //   of which in FAR rows
+    long long n_atom_segments;          // ATOM mode: list segments summed over blocks
     int atom_bad;                       // 1: ATOM lists unusable (capacity / too many chunks): CLUSTER is used
     int pad1;
     // PCG scalars
@@ -105,6 +107,11 @@ struct Ctx {
     int part_cap;           // >= the largest grid of any reducing kernel (n_blocks + MAX_PARTIALS)
     double *h_scalars;      // pinned host scratch (8 doubles) for scalar read-backs
     double *h_ring, *d_ring; // mapped pinned ring: |r|^2 of each PCG iteration, written by the device
+    // ATOM lists: far class (atom_pairs.cu atom_far_setup)
+    bool far_on;            // false: FP64 mode or beta = 0, every pair takes the full formula
+    double far_x0;          // a pair is FAR iff x = R^3 w_i w_j >= far_x0 and R >= far_rmin
+    double far_rmin;
+    float far_q[6];         // far fit of erfcx in t = 1/R
     bool fuse_q;            // ATOM-mode T.mu kernel also forms q = p/alpha - T p - self p and p.q (PCG)
     int spec_iter;          // >= 0: the pair kernel about to be launched belongs to PCG iteration spec_iter
     DeviceState *h_state;   // pinned host copy of *st (list header), valid when header_valid
@@ -176,6 +183,10 @@ int cluster_tmatvec(Ctx *c, cudaStream_t s);
 int cluster_field(Ctx *c, cudaStream_t s);
 long long cluster_slots(Ctx *c);
 int atom_build(Ctx *c, cudaStream_t s);
+void atom_far_setup(Ctx *c);
+int atom_lists_configure(Ctx *c);
+int atom_pairs_configure(Ctx *c);
+int cluster_pairs_configure(Ctx *c);
 int atom_tmatvec(Ctx *c, cudaStream_t s);
 int atom_field(Ctx *c, cudaStream_t s);
 long long atom_slots(Ctx *c);
