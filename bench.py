@@ -14,7 +14,7 @@ pair {i,j} with R <= r_c evaluated once, for both atoms, in the field or in one 
 A step performs N_pair * (1 + n_matvec) of them (n_matvec = PCG iterations + 1 for the initial
 residual); value = that / step time, summed over GPUs (replicas: SURVEY 8(e) "replicas only").
 
-Prints ONE JSON line on rank 0 (see DESIGN.md section 8 for every key).
+Prints ONE JSON line on rank 0 (see DESIGN.md section 7 for every key).
 """
 from __future__ import annotations
 
@@ -38,14 +38,16 @@ METRIC = "useful pair interactions/s (field + T.mu matvecs of one list-build + f
 UNIT = "pair interactions/s"
 FLOPS_PER_PAIR_TMU = 89      # 32 FFMA*2 + 22 FMUL + 3 FADD per evaluated slot
 FLOPS_PER_PAIR_FIELD = 160
-# What the ATOM-list MIXED T.mu kernel EXECUTES per evaluated slot (ordered pair), counted in the SASS
-# of its inner loop (8 slots per trip: 76 FFMA2 + 40 FMUL2 + 8 FADD2 + 51 FFMA + 24 FMUL, DESIGN.md
-# section 5.3): FMA-pipe lane-cycles (a packed instruction holds the pipe 2 cycles) and FP32 flops.
-TMU_ATOM_MIXED_PIPE_CYCLES_PER_SLOT = (2 * (76 + 40 + 8) + 51 + 24) / 8
-TMU_ATOM_MIXED_FLOPS_PER_SLOT = (4 * 76 + 2 * 40 + 2 * 8 + 2 * 51 + 24) / 8
-# ALU roofline denominator derived in DESIGN.md section 7: 148 SMs x 128 FP32 lanes x 2 flop x 1.965 GHz
-PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-PEAK_FP64_TFLOPS = PEAK_FP32_TFLOPS / 2
+# What the ATOM-list MIXED T.mu loop EXECUTES per evaluated slot (ordered pair), counted in the SASS of
+# its rows (8 slots per row and lane) -- profiles/r02_sass_tmu_rows.txt, build named there:
+#   FAR row : 44 FFMA2 + 24 FMUL2 + 8 FADD2 + 48 FFMA + 16 FMUL + 8 FADD, 16 MUFU
+#   NEAR row: 68 FFMA2 + 44 FMUL2 + 8 FADD2 + 48 FFMA + 24 FMUL + 8 FADD, 32 MUFU
+# FMA-pipe lane-cycles (a packed instruction holds the pipe 2 cycles) and FP32 flops per slot:
+TMU_FAR_PIPE_CYCLES = (2 * (44 + 24 + 8) + 48 + 16 + 8) / 8
+TMU_NEAR_PIPE_CYCLES = (2 * (68 + 44 + 8) + 48 + 24 + 8) / 8
+TMU_FAR_FLOPS = (4 * 44 + 2 * 24 + 2 * 8 + 2 * 48 + 16 + 8) / 8
+TMU_NEAR_FLOPS = (4 * 68 + 2 * 44 + 2 * 8 + 2 * 48 + 24 + 8) / 8
+FP32_LANES_PER_SM = 128      # B200_PROFILING.md unit counts; FP64: half rate
 WORKLOADS = {0: "cfg0_water648", 1: "cfg1_dhfr_size_23559", 2: "cfg2_hetero_98304", 3: "cfg3_stmv_size_1066629"}
 
 
@@ -232,8 +234,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
           for _ in range(args.steps)]
     sampler = ClockSampler(local_rank)
     pk.tkhp_profile_reset(P.ctx, True)
-    prof_tot = dict(launches=0, n_tmatvec=0, tmatvec_ms=0.0, n_field=0, field_ms=0.0)
-    iters = []
+    prof_tot = dict(launches=0, n_tmatvec=0, tmatvec_ms=0.0, n_field=0, field_ms=0.0,
+                    n_solve=0, solve_ms=0.0, solve_matvecs=0)
+    iters, phases = [], []
     sampler.start()
     barrier()
     t_wall0 = time.perf_counter()
@@ -244,13 +247,14 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         ev[k][1].record(stream)
         iters.append(it)
         pr = pk.tkhp_profile_read(P.ctx)
+        pr.update(pk.tkhp_profile_read_solve(P.ctx))
         for key in prof_tot:
             prof_tot[key] += pr[key]
+        phases.append(P.timings())
         pk.tkhp_profile_reset(P.ctx, True)
     barrier()
     wall_s = time.perf_counter() - t_wall0
     clocks = sampler.stop()
-    phase_ms = P.timings()
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = sum(step_ms)
     total_ms, wall_s = replicas.max_over_ranks([total_ms, wall_s], dist, dev)
@@ -261,36 +265,113 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     pairs_per_step = n_pair * (1 + n_matvec)
     value = replicas.aggregate_throughput(pairs_per_step, world, ms_per_step)
 
-    # ---- dominant kernel roofline (T.mu pair kernel), measured live with CUDA events
-    tmu_ms = prof_tot["tmatvec_ms"] / max(prof_tot["n_tmatvec"], 1)
+    def stats(v):
+        return {"mean": statistics.mean(v), "median": statistics.median(v), "min": min(v)}
+    phase_names = ["build", "field", "tmatvec", "solve", "energy"]
+    phase_ms = {nm: statistics.mean(ph[nm] for ph in phases) for nm in phase_names}
+    phase_stats = {nm: stats([ph[nm] for ph in phases]) for nm in phase_names if nm != "tmatvec"}
+
+    # ---- a stand-alone T.mu product (tkhp_tmatvec: pack + pair kernel + finish), 20 calls, L2 flushed
+    d_probe = torch.as_tensor(np.random.default_rng(5).standard_normal((n, 3)) * 0.1, dtype=f64, device=dev)
+    d_out = torch.empty((n, 3), dtype=f64, device=dev)
+    for _ in range(3):
+        pk.tkhp_tmatvec(P.ctx, d_probe, d_out, stream)
+    pk.tkhp_profile_reset(P.ctx, True)
+    mv_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+    for a_, b_ in mv_ev:
+        flush.fill_(1)
+        a_.record(stream)
+        pk.tkhp_tmatvec(P.ctx, d_probe, d_out, stream)
+        b_.record(stream)
+    torch.cuda.synchronize()
+    mv_call = [a_.elapsed_time(b_) for a_, b_ in mv_ev]
+    mv_prof = pk.tkhp_profile_read(P.ctx)
+    mv_kernel_ms = mv_prof["tmatvec_ms"] / max(mv_prof["n_tmatvec"], 1)
+    phase_ms["tmatvec"] = statistics.median(mv_call)
+    phase_stats["tmatvec"] = stats(mv_call)
+    pk.tkhp_profile_reset(P.ctx, False)
+
+    # ---- dominant kernel roofline, measured live with CUDA events on the library's stream
+    props = torch.cuda.get_device_properties(dev)
+    sm_count = props.multi_processor_count
+    sm_ghz = 1.965
+    try:
+        sm_ghz = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["sm_max_mhz"] / 1e3
+    except Exception:
+        if clocks.get("sm_max_mhz"):
+            sm_ghz = clocks["sm_max_mhz"] / 1e3
+    lanes_per_s = sm_count * FP32_LANES_PER_SM * sm_ghz * 1e9
+    peak32 = 2 * lanes_per_s / 1e12
+    peak = peak32 if args.precision == "mixed" else peak32 / 2
     fld_ms = prof_tot["field_ms"] / max(prof_tot["n_field"], 1)
-    peak = PEAK_FP32_TFLOPS if args.precision == "mixed" else PEAK_FP64_TFLOPS
-    achieved = FLOPS_PER_PAIR_TMU * n_pair / (tmu_ms * 1e-3) / 1e12
-    executed = FLOPS_PER_PAIR_TMU * n_slots / (tmu_ms * 1e-3) / 1e12
+    persistent = prof_tot["n_solve"] > 0
+    if persistent:
+        # the whole solve is ONE launch of k_pcg_persist: its T.mu products are the algorithmic work
+        kern_ms = prof_tot["solve_ms"] / prof_tot["n_solve"]
+        mv_per_launch = prof_tot["solve_matvecs"] / prof_tot["n_solve"]
+        kernel_name = "k_pcg_persist (whole PCG solve: %.1f T.mu products + vector updates, one cooperative launch)" % mv_per_launch
+        share = prof_tot["solve_ms"] / total_ms if world == 1 else None
+        n_timed = prof_tot["n_solve"]
+    else:
+        kern_ms = prof_tot["tmatvec_ms"] / max(prof_tot["n_tmatvec"], 1)
+        mv_per_launch = 1.0
+        kernel_name = "T.mu pair kernel (%s list)" % mode_name[mode_in_use]
+        share = prof_tot["tmatvec_ms"] / total_ms if world == 1 else None
+        n_timed = prof_tot["n_tmatvec"]
+    alg_flops = FLOPS_PER_PAIR_TMU * n_pair * mv_per_launch
+    achieved = alg_flops / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0
     roofline = {
-        "bound": "alu", "kernel": "T.mu pair kernel (%s list)" % mode_name[mode_in_use],
+        "bound": "alu", "kernel": kernel_name,
         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
         "traffic": None,
-        "algorithmic_flops_per_launch": FLOPS_PER_PAIR_TMU * n_pair,
-        "avg_launch_ms": tmu_ms, "launches_timed": prof_tot["n_tmatvec"],
-        "share_of_step": prof_tot["tmatvec_ms"] / total_ms if world == 1 else None,
-        "executed_slots_per_launch": n_slots, "executed_tflops_nominal": executed,
-        "executed_frac_of_peak": executed / peak,
-        "useful_pairs_per_s_kernel": n_pair / (tmu_ms * 1e-3),
+        "algorithmic_flops_per_launch": alg_flops, "matvecs_per_launch": mv_per_launch,
+        "avg_launch_ms": kern_ms, "ms_per_matvec_in_kernel": kern_ms / mv_per_launch, "launches_timed": n_timed,
+        "share_of_step": share,
+        "executed_slots_per_matvec": n_slots,
+        "useful_pairs_per_s_kernel": n_pair * mv_per_launch / (kern_ms * 1e-3) if kern_ms > 0 else 0.0,
         "field_kernel_avg_ms": fld_ms,
-        "peak_note": "148 SM x 128 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
+        "field_kernel_tflops": FLOPS_PER_PAIR_FIELD * n_pair / (fld_ms * 1e-3) / 1e12 if fld_ms > 0 else None,
+        "peak_note": "%d SMs (queried) x %d FP32 lanes x 2 flop x %.3f GHz (MEASURED_PEAKS sm_max_mhz; DESIGN.md section 6)"
+                     % (sm_count, FP32_LANES_PER_SM, sm_ghz),
+        "standalone_tmatvec": {
+            "kernel": "T.mu pair kernel (%s list), one launch per product" % mode_name[mode_in_use],
+            "avg_kernel_ms": mv_kernel_ms, "launches_timed": mv_prof["n_tmatvec"],
+            "achieved": FLOPS_PER_PAIR_TMU * n_pair / (mv_kernel_ms * 1e-3) / 1e12 if mv_kernel_ms > 0 else None,
+            "frac": FLOPS_PER_PAIR_TMU * n_pair / (mv_kernel_ms * 1e-3) / 1e12 / peak if mv_kernel_ms > 0 else None,
+            "call_ms": phase_stats["tmatvec"],
+        },
     }
     if mode_in_use == pk.TKHP_LIST_ATOM and args.precision == "mixed":
-        lanes_per_s = 148 * 128 * 1.965e9
-        roofline["executed_flops_per_slot_sass"] = TMU_ATOM_MIXED_FLOPS_PER_SLOT
-        roofline["executed_tflops_sass"] = TMU_ATOM_MIXED_FLOPS_PER_SLOT * n_slots / (tmu_ms * 1e-3) / 1e12
-        roofline["fma_pipe_busy_frac"] = TMU_ATOM_MIXED_PIPE_CYCLES_PER_SLOT * n_slots / (tmu_ms * 1e-3) / lanes_per_s
+        far, near, segs, far_on = P.nblist_atom_stats()
+        if not far_on:
+            near, far = far + near, 0
+        pipe_cycles = TMU_FAR_PIPE_CYCLES * far + TMU_NEAR_PIPE_CYCLES * near
+        flops_sass = TMU_FAR_FLOPS * far + TMU_NEAR_FLOPS * near
+        roofline["executed_far_slots"] = far
+        roofline["executed_near_slots"] = near
+        roofline["executed_tflops_sass"] = flops_sass * mv_per_launch / (kern_ms * 1e-3) / 1e12
+        roofline["fma_pipe_busy_frac"] = pipe_cycles * mv_per_launch / (kern_ms * 1e-3) / lanes_per_s
+        roofline["sass_counts_from"] = "profiles/r02_sass_tmu_rows.txt"
     try:
         traffic_file = ROOT / "profiles" / "traffic.json"
         if traffic_file.exists():
-            roofline["traffic"] = json.loads(traffic_file.read_text()).get(mode_name[mode_in_use])
+            tj = json.loads(traffic_file.read_text())
+            roofline["traffic"] = tj.get("k_pcg_persist" if persistent else mode_name[mode_in_use])
+            roofline["traffic_note"] = tj.get("note")
     except Exception:
         pass
+    # list build against the HBM roofline (~190 B/atom of prescribed traffic + the lists written)
+    hbm_gbs = None
+    try:
+        hbm_gbs = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"]
+    except Exception:
+        pass
+    build_bytes = 190.0 * n + 2.0 * n_slots
+    build_roofline = {"bound": "hbm", "algorithmic_bytes": build_bytes, "ms": phase_ms["build"],
+                      "achieved_gbs": build_bytes / (phase_ms["build"] * 1e-3) / 1e9 if phase_ms["build"] > 0 else None,
+                      "peak_gbs": hbm_gbs,
+                      "frac": (build_bytes / (phase_ms["build"] * 1e-3) / 1e9 / hbm_gbs) if hbm_gbs and phase_ms["build"] > 0 else None,
+                      "note": "190 B/atom (SURVEY 8(d)) + 2 B per list slot written"}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
@@ -344,7 +425,6 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     if roofline is not None and fma_peak:
         roofline["peak_measured_fma_chain"] = fma_peak
         roofline["frac_of_measured_fma"] = achieved / fma_peak
-        roofline["executed_frac_of_measured_fma"] = executed / fma_peak
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -358,7 +438,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                    "parallelism": "replicas x%d" % world, "l2": "flushed between timed steps (256 MiB fill)"},
         "n_pair_within_cutoff": n_pair, "pcg_iterations": statistics.mean(iters),
         "pair_interactions_per_step": pairs_per_step, "energy_kcal_mol": energy, "final_rms": rms,
-        "phase_ms": phase_ms,
+        "phase_ms": phase_ms, "phase_ms_stats": phase_stats, "step_ms_stats": stats(step_ms),
+        "build_roofline": build_roofline,
+        "launch_bound": n < 5000,
         "wall_ms_per_step_incl_flush": 1e3 * wall_s / args.steps,
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": prof_tot["launches"], "clocks": clocks,

@@ -85,7 +85,16 @@ typedef struct {
     int32_t max_stage_per_chunk; /* ATOM mode: staged atoms per shared-memory chunk (multiple of 32);
                                     0 = automatic (what fits the kernel's shared memory); tests use a
                                     small value to exercise the multi-chunk path */
+    int32_t solver_flags;        /* OR of TKHP_SOLVER_*; 0 = automatic (tests use the flags to force the
+                                    fall-back paths of tkhp_polar_solve) */
+    int32_t reserved;            /* must be 0 */
 } tkhp_params;
+
+/* tkhp_params.solver_flags */
+enum {
+    TKHP_SOLVER_NO_PERSISTENT = 1, /* never run the solve as one persistent cooperative kernel */
+    TKHP_SOLVER_NO_FUSED_STEP = 2  /* launch-per-matvec path: update and direction as two kernels */
+};
 
 /* Bytes of device workspace tkhp_create() needs for these parameters.  Host, pure. */
 int tkhp_workspace_bytes(const tkhp_params *params, size_t *bytes);
@@ -207,6 +216,10 @@ int tkhp_last_timings(tkhp_ctx *ctx, double ms[5]);
 int tkhp_profile_reset(tkhp_ctx *ctx, int32_t enable_kernel_events);
 int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmatvec_kernels,
                       double *tmatvec_kernel_ms, int32_t *n_field_kernels, double *field_kernel_ms);
+/* The same for the persistent PCG kernel (MIXED precision, ATOM lists: the whole solve is one
+ * cooperative launch): recorded launches since the reset, their summed
+ * duration in ms and the T.mu products they performed (iterations + 1 per solve). */
+int tkhp_profile_read_solve(tkhp_ctx *ctx, int32_t *n_solve_kernels, double *solve_kernel_ms, int64_t *n_matvecs);
 
 /*
  * Register-resident FMA microbenchmark used as the measured ALU roofline denominator

@@ -10,18 +10,20 @@ but creating a context without a CUDA device raises, and a missing
 ``libtkhp.so`` raises at import of :mod:`paper_2011_01207_b200.binding`.
 """
 from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM,
+                      TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP,
                       TkhpError, TkhpParams, Polarizer, lib, lib_path,
                       tkhp_workspace_bytes, tkhp_create, tkhp_destroy, tkhp_last_error,
                       tkhp_nblist_build, tkhp_nblist_view, tkhp_nblist_stats, tkhp_nblist_atom_stats,
                       tkhp_perm_field, tkhp_tmatvec, tkhp_polar_solve,
                       tkhp_polar_energy, tkhp_polarize_host, tkhp_last_timings,
-                      tkhp_fma_peak, tkhp_profile_reset, tkhp_profile_read, EXPORTED_SYMBOLS)
+                      tkhp_fma_peak, tkhp_profile_reset, tkhp_profile_read, tkhp_profile_read_solve,
+                      EXPORTED_SYMBOLS)
 
 __all__ = [
-    "TKHP_FP64", "TKHP_MIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TKHP_LIST_ATOM", "TkhpError",
+    "TKHP_FP64", "TKHP_MIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TKHP_LIST_ATOM", "TKHP_SOLVER_NO_PERSISTENT", "TKHP_SOLVER_NO_FUSED_STEP", "TkhpError",
     "TkhpParams", "Polarizer", "lib", "lib_path", "tkhp_workspace_bytes", "tkhp_create",
     "tkhp_destroy", "tkhp_last_error", "tkhp_nblist_build", "tkhp_nblist_view",
     "tkhp_nblist_stats", "tkhp_nblist_atom_stats", "tkhp_perm_field", "tkhp_tmatvec", "tkhp_polar_solve",
     "tkhp_polar_energy", "tkhp_polarize_host", "tkhp_last_timings", "tkhp_fma_peak",
-    "tkhp_profile_reset", "tkhp_profile_read", "EXPORTED_SYMBOLS",
+    "tkhp_profile_reset", "tkhp_profile_read", "tkhp_profile_read_solve", "EXPORTED_SYMBOLS",
 ]

@@ -11,6 +11,7 @@ TKHP_EINVAL, TKHP_ECUDA, TKHP_ECUTOFF, TKHP_ENOLIST = -1, -2, -3, -4
 TKHP_ENOCONV, TKHP_ECAPACITY, TKHP_ENONFINITE = -5, -6, -7
 TKHP_FP64, TKHP_MIXED = 0, 1
 TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM = 0, 1, 2
+TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP = 1, 2
 
 _ERR_NAMES = {-1: "TKHP_EINVAL", -2: "TKHP_ECUDA", -3: "TKHP_ECUTOFF", -4: "TKHP_ENOLIST",
               -5: "TKHP_ENOCONV", -6: "TKHP_ECAPACITY", -7: "TKHP_ENONFINITE"}
@@ -20,6 +21,7 @@ EXPORTED_SYMBOLS = [
     "tkhp_nblist_build", "tkhp_nblist_view", "tkhp_nblist_stats", "tkhp_nblist_atom_stats", "tkhp_perm_field",
     "tkhp_tmatvec", "tkhp_polar_solve", "tkhp_polar_energy", "tkhp_polarize_host",
     "tkhp_last_timings", "tkhp_fma_peak", "tkhp_profile_reset", "tkhp_profile_read",
+    "tkhp_profile_read_solve",
 ]
 
 
@@ -35,7 +37,8 @@ class TkhpParams(Structure):
                 ("list_mode", c_int32), ("box", c_double), ("cutoff", c_double),
                 ("skin", c_double), ("ewald_beta", c_double), ("thole_a", c_double),
                 ("max_tiles_per_block", c_int32), ("max_nbrs_per_cluster", c_int32),
-                ("max_nbrs_per_atom", c_int32), ("max_stage_per_chunk", c_int32)]
+                ("max_nbrs_per_atom", c_int32), ("max_stage_per_chunk", c_int32),
+                ("solver_flags", c_int32), ("reserved", c_int32)]
 
 
 def lib_path() -> Path:
@@ -79,6 +82,7 @@ def lib() -> ctypes.CDLL:
         L.tkhp_profile_reset.argtypes = [c_void_p, c_int32]
         L.tkhp_profile_read.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int32),
                                         POINTER(c_double), POINTER(c_int32), POINTER(c_double)]
+        L.tkhp_profile_read_solve.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_double), POINTER(c_int64)]
         for name in EXPORTED_SYMBOLS:
             if name != "tkhp_last_error":
                 getattr(L, name).restype = ctypes.c_int
@@ -226,6 +230,13 @@ def tkhp_profile_read(ctx):
                 field_ms=tf.value)
 
 
+def tkhp_profile_read_solve(ctx):
+    """-> dict(n_solve, solve_ms, solve_matvecs) of the persistent PCG kernel."""
+    n, ms, mv = c_int32(0), c_double(0.0), c_int64(0)
+    _check(lib().tkhp_profile_read_solve(ctx, byref(n), byref(ms), byref(mv)), ctx)
+    return dict(n_solve=n.value, solve_ms=ms.value, solve_matvecs=mv.value)
+
+
 def tkhp_fma_peak(device: int, precision: int, seconds: float = 2.0) -> float:
     out = c_double(0.0)
     _check(lib().tkhp_fma_peak(device, precision, seconds, byref(out)))
@@ -243,7 +254,7 @@ class Polarizer:
     def __init__(self, n_atoms, box, cutoff=7.0, skin=2.0, ewald_beta=0.5446, thole_a=0.39,
                  precision=TKHP_MIXED, list_mode=TKHP_LIST_TILES, device=0,
                  max_tiles_per_block=0, max_nbrs_per_cluster=0, max_nbrs_per_atom=0,
-                 max_stage_per_chunk=0):
+                 max_stage_per_chunk=0, solver_flags=0):
         import torch
         if not torch.cuda.is_available():
             raise TkhpError(TKHP_ECUDA, "no CUDA device: libtkhp has no CPU fallback")
@@ -251,7 +262,7 @@ class Polarizer:
         self.device = torch.device("cuda", device)
         self.params = TkhpParams(n_atoms, precision, device, list_mode, box, cutoff, skin,
                                  ewald_beta, thole_a, max_tiles_per_block, max_nbrs_per_cluster,
-                                 max_nbrs_per_atom, max_stage_per_chunk)
+                                 max_nbrs_per_atom, max_stage_per_chunk, solver_flags, 0)
         self.n = n_atoms
         nbytes = tkhp_workspace_bytes(self.params)
         with torch.cuda.device(self.device):

@@ -34,6 +34,7 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
     }
     if (p->precision == TKHP_MIXED && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }
     if (p->max_tiles_per_block < 0 || p->max_nbrs_per_cluster < 0 || p->max_nbrs_per_atom < 0) { snprintf(err, n, "negative capacity"); return TKHP_EINVAL; }
+    if (p->solver_flags & ~(TKHP_SOLVER_NO_PERSISTENT | TKHP_SOLVER_NO_FUSED_STEP) || p->reserved != 0) { snprintf(err, n, "unknown solver_flags / non-zero reserved field"); return TKHP_EINVAL; }
     if (p->max_stage_per_chunk < 0 || (p->max_stage_per_chunk & 31)) { snprintf(err, n, "max_stage_per_chunk must be a non-negative multiple of 32"); return TKHP_EINVAL; }
     return TKHP_OK;
 }
@@ -105,6 +106,7 @@ static size_t carve(Ctx *c, const tkhp_params *p, void *base) {
     o->pairs = w.take<int2>((size_t)cap_tiles);
     o->acc = w.take<double>(3 * n_pad);
     o->mu32 = f64 ? nullptr : w.take<float4>(n_pad);
+    o->u32 = f64 ? nullptr : w.take<float4>(n_pad);
     o->mu64 = f64 ? w.take<double4>(n_pad) : nullptr;
     o->mp32 = f64 ? nullptr : w.take<float4>(3 * n_pad);
     o->mp64 = f64 ? w.take<double4>(3 * n_pad) : nullptr;
@@ -196,7 +198,9 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     if (cudaGetDeviceProperties(&prop, params->device) != cudaSuccess) { delete c; return TKHP_ECUDA; }
     c->sm_count = prop.multiProcessorCount;
     atom_far_setup(c);
-    if (cluster_pairs_configure(c) || atom_lists_configure(c) || atom_pairs_configure(c)) {
+    c->no_persist = (params->solver_flags & TKHP_SOLVER_NO_PERSISTENT) != 0;
+    c->no_fused_step = (params->solver_flags & TKHP_SOLVER_NO_FUSED_STEP) != 0;
+    if (cluster_pairs_configure(c) || atom_lists_configure(c) || atom_pairs_configure(c) || atom_solve_configure(c)) {
         snprintf(g_create_err, sizeof(g_create_err), "%s", c->err);
         delete c;
         return TKHP_ECUDA;
@@ -216,7 +220,7 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     for (int i = 0; i < 10; ++i) cudaEventCreate(&c->ev[i]);
     cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
     for (int i = 0; i < 2; ++i) cudaEventCreateWithFlags(&c->copy_ev[i], cudaEventDisableTiming);
-    for (int w = 0; w < 2; ++w)
+    for (int w = 0; w < 3; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventCreate(&c->prof_ev[w][i]);
     for (int i = 0; i < 5; ++i) c->last_ms[i] = -1.0;
     c->built = false;
@@ -235,7 +239,7 @@ int tkhp_destroy(tkhp_ctx *ctx) {
     for (int i = 0; i < 10; ++i) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 2; ++i) cudaEventDestroy(c->copy_ev[i]);
     cudaStreamDestroy(c->copy_stream);
-    for (int w = 0; w < 2; ++w)
+    for (int w = 0; w < 3; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventDestroy(c->prof_ev[w][i]);
     cudaFreeHost(c->h_ring);
     cudaFreeHost(c->h_scalars);
@@ -425,7 +429,8 @@ int tkhp_profile_reset(tkhp_ctx *ctx, int32_t enable_kernel_events) {
     c->n_launches = 0;
     c->n_noop_launches = 0;
     c->prof = enable_kernel_events != 0;
-    c->prof_n[0] = c->prof_n[1] = 0;
+    c->prof_n[0] = c->prof_n[1] = c->prof_n[2] = 0;
+    c->prof_solve_matvecs = 0;
     return TKHP_OK;
 }
 
@@ -453,6 +458,25 @@ int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmat
     if (tmatvec_kernel_ms) *tmatvec_kernel_ms = tot[0];
     if (n_field_kernels) *n_field_kernels = cnt[1];
     if (field_kernel_ms) *field_kernel_ms = tot[1];
+    return TKHP_OK;
+}
+
+int tkhp_profile_read_solve(tkhp_ctx *ctx, int32_t *n_solve_kernels, double *solve_kernel_ms, int64_t *n_matvecs) {
+    if (!ctx) return TKHP_EINVAL;
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    double tot = 0.0;
+    for (int i = 0; i < c->prof_n[2]; ++i) {
+        float t = 0.f;
+        if (cudaEventSynchronize(c->prof_ev[2][2 * i + 1]) != cudaSuccess ||
+            cudaEventElapsedTime(&t, c->prof_ev[2][2 * i], c->prof_ev[2][2 * i + 1]) != cudaSuccess) {
+            cudaGetLastError();
+            return set_err(c, TKHP_ECUDA, "profile events not complete%s");
+        }
+        tot += t;
+    }
+    if (n_solve_kernels) *n_solve_kernels = c->prof_n[2];
+    if (solve_kernel_ms) *solve_kernel_ms = tot;
+    if (n_matvecs) *n_matvecs = c->prof_solve_matvecs;
     return TKHP_OK;
 }
 

@@ -101,7 +101,9 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int L8 = L >> 3;                                                                                   // L is a multiple of 8
     uint4 *__restrict__ rows = reinterpret_cast<uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;    // row r of this lane: rows[r * 32]
     const int rows_cap = ws.a_cap >> 3;
-    const unsigned dummy = (unsigned)s_chunk * (unsigned)sizeof(vec4);
+    // padding entries point at the record after the largest chunk of THIS group (the kernels put a
+    // far-away record with zero payload there)
+    const unsigned dummy = (unsigned)atom_dummy_index(count, n_chunks) * (unsigned)sizeof(vec4);
     const unsigned l16 = (unsigned)lane & 15u;
     const int fcap = ws.far_cap, fcol = fcap >> 4, ncol = NEAR_CAP >> 4;
     uint16_t *img_f = reinterpret_cast<uint16_t *>(smem_raw + (size_t)s_chunk * sizeof(vec4)) +

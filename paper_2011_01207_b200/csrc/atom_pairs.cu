@@ -187,7 +187,7 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
     constexpr int SU = sizeof(real) == 8 ? 4 : 8;   // staged records in flight per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk + 1], last = dummy
+    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk + 1]; the dummy follows the group's largest chunk
     vec4 *s_pay = s_pos + (s_chunk + 1);                       // NPAY arrays of [s_chunk + 1]
     const int pstride = s_chunk + 1;
     const int pay_stride = pstride * (int)sizeof(vec4);
@@ -217,8 +217,9 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         vec4 far, zero;
         far.x = far.y = far.z = (real)(-2.0f * PHANTOM_FAR); far.w = 0;
         zero.x = zero.y = zero.z = zero.w = 0;
-        s_pos[s_chunk] = far;
-        for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + s_chunk] = zero;
+        const int dmy = atom_dummy_index(count, n_chunks);
+        s_pos[dmy] = far;
+        for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + dmy] = zero;
     }
 
     // My rows are part, part + wpb, ... of the block's row stream, whatever segment they fall in; a
@@ -302,7 +303,7 @@ k_atom_tmu32(ClusterWs ws, const float4 *__restrict__ gpos, const float4 *__rest
     if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     constexpr int SU = 4;                              // staged records in flight per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int pstride = s_chunk + 1;                   // last record = dummy
+    const int pstride = s_chunk + 1;                   // the dummy record follows the group's largest chunk
     float4 *s_a = reinterpret_cast<float4 *>(smem_raw);
     float2 *s_b = reinterpret_cast<float2 *>(smem_raw + (size_t)16 * pstride);
     float *s_w = reinterpret_cast<float *>(smem_raw + (size_t)24 * pstride);
@@ -335,25 +336,15 @@ k_atom_tmu32(ClusterWs ws, const float4 *__restrict__ gpos, const float4 *__rest
 
     if (t == 0) {                              // permanent dummy record: far away, zero payload
         const float far = -2.0f * PHANTOM_FAR;
-        s_a[s_chunk] = make_float4(far, far, far, 0.f);
-        s_b[s_chunk] = make_float2(0.f, 0.f);
-        s_w[s_chunk] = 0.f;
+        const int dmy = atom_dummy_index(count, n_chunks);
+        s_a[dmy] = make_float4(far, far, far, 0.f);
+        s_b[dmy] = make_float2(0.f, 0.f);
+        s_w[dmy] = 0.f;
     }
 
-    // Row stream: my rows are part, part + wpb, ... of the block's rows, whatever segment they fall
-    // in.  A row (16 bytes per lane) is loaded into registers two rows before its use.
     const int t_total = (active && n_chunks <= NCH_MAX) ? seg_row0(seg[NSEG_MAX - 1]) : 0;
-    int n_load = t_total > part ? (t_total - part + wpb - 1) / wpb : 0;       // my rows not yet requested
-    const uint4 *rp = reinterpret_cast<const uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane + (size_t)part * 32;
-    uint4 e1 = make_uint4(0, 0, 0, 0), e2 = e1;
-    if (n_load > 0) { e1 = ldg_row(rp); rp += 32 * wpb; --n_load; }
-    if (n_load > 0) { e2 = ldg_row(rp); rp += 32 * wpb; --n_load; }
-    auto next_row = [&]() {
-        const uint4 e = e1;
-        e1 = e2;
-        if (n_load > 0) { e2 = ldg_row(rp); rp += 32 * wpb; --n_load; }
-        return e;
-    };
+    RowStream R;
+    R.open(reinterpret_cast<const uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane, t_total, part, wpb);
 
     int d = 0, n_rows = 0;
     int2 sd = seg[0];
@@ -393,34 +384,7 @@ k_atom_tmu32(ClusterWs ws, const float4 *__restrict__ gpos, const float4 *__rest
 #ifdef TKHP_DBG_NOLOOP
         continue;
 #endif
-        while (seg_chunk(sd) == c) {
-            const int row0 = seg_row0(sd);
-            const int ncf = seg_far_calls(sd), ncn = seg_near_calls(sd);
-            // first class of rows (FAR pairs, or every pair when the far class is off)
-            const int f_full = row0 + (ncf >> 2);
-            for (; tg < f_full; tg += wpb) {
-                const uint4 e = next_row();
-                tmu_row<FAR>(S, e, 4, L, K, A);
-                if ((++n_rows & 3) == 0) A.flush(dx, dy, dz);   // every 32 entries: FP32 partial -> FP64
-            }
-            if ((ncf & 3) && tg == f_full) {
-                const uint4 e = next_row();
-                tmu_row<FAR>(S, e, ncf & 3, L, K, A);
-                tg += wpb;
-            }
-            const int n0 = row0 + ((ncf + 3) >> 2), n_full = n0 + (ncn >> 2);
-            for (; tg < n_full; tg += wpb) {
-                const uint4 e = next_row();
-                tmu_row<false>(S, e, 4, L, K, A);
-                if ((++n_rows & 3) == 0) A.flush(dx, dy, dz);
-            }
-            if ((ncn & 3) && tg == n_full) {
-                const uint4 e = next_row();
-                tmu_row<false>(S, e, ncn & 3, L, K, A);
-                tg += wpb;
-            }
-            sd = seg[++d];
-        }
+        tmu_walk<FAR>(seg, c, d, sd, tg, wpb, R, S, L, K, A, n_rows, dx, dy, dz);
     }
     A.flush(dx, dy, dz);
     pair_epilogue<true>(smem_raw, dx, dy, dz, wpb, part, active, slot, n_pad, acc, st, fuse);

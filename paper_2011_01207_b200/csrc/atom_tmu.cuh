@@ -166,4 +166,63 @@ __device__ __forceinline__ uint4 ldg_row(const uint4 *p) {
 // part + wpb, ... and the parts are added in a fixed order at the end (bit-reproducible)
 __device__ __forceinline__ int warps_per_block(int nb) { return nb >= 5 ? 1 : (nb >= 3 ? 2 : (nb == 2 ? 4 : 8)); }
 
+// A warp's stream of list rows: my rows are part, part + wpb, ... of the block's rows, whatever
+// segment they fall in.  A row (16 bytes per lane) is loaded into registers two rows before its use.
+struct RowStream {
+    const uint4 *rp;
+    int n_load, step;
+    uint4 e1, e2;
+    __device__ __forceinline__ void open(const uint4 *rows_of_lane, int t_total, int part, int wpb) {
+        n_load = t_total > part ? (t_total - part + wpb - 1) / wpb : 0;       // my rows not yet requested
+        rp = rows_of_lane + (size_t)part * 32;
+        step = 32 * wpb;
+        e1 = make_uint4(0, 0, 0, 0);
+        e2 = e1;
+        if (n_load > 0) { e1 = ldg_row(rp); rp += step; --n_load; }
+        if (n_load > 0) { e2 = ldg_row(rp); rp += step; --n_load; }
+    }
+    __device__ __forceinline__ uint4 next() {
+        const uint4 e = e1;
+        e1 = e2;
+        if (n_load > 0) { e2 = ldg_row(rp); rp += step; --n_load; }
+        return e;
+    }
+};
+
+// All segments of chunk c of one block: FAR rows, then NEAR rows, of every segment.  `tg` is my next
+// row, (sd, d) the descriptor cursor; FP32 partials go to the FP64 registers every 4 rows.
+template <bool FAR>
+__device__ __forceinline__ void tmu_walk(const int2 *__restrict__ seg, int c, int &d, int2 &sd, int &tg, int wpb,
+                                         RowStream &R, const TmuSmem &S, const TmuLane &L, const TmuConsts &K,
+                                         PartialTmu &A, int &n_rows, double &dx, double &dy, double &dz) {
+    while (seg_chunk(sd) == c) {
+        const int row0 = seg_row0(sd);
+        const int ncf = seg_far_calls(sd), ncn = seg_near_calls(sd);
+        // first class of rows (FAR pairs, or every pair when the far class is off)
+        const int f_full = row0 + (ncf >> 2);
+        for (; tg < f_full; tg += wpb) {
+            const uint4 e = R.next();
+            tmu_row<FAR>(S, e, 4, L, K, A);
+            if ((++n_rows & 3) == 0) A.flush(dx, dy, dz);   // every 32 entries: FP32 partial -> FP64
+        }
+        if ((ncf & 3) && tg == f_full) {
+            const uint4 e = R.next();
+            tmu_row<FAR>(S, e, ncf & 3, L, K, A);
+            tg += wpb;
+        }
+        const int n0 = row0 + ((ncf + 3) >> 2), n_full = n0 + (ncn >> 2);
+        for (; tg < n_full; tg += wpb) {
+            const uint4 e = R.next();
+            tmu_row<false>(S, e, 4, L, K, A);
+            if ((++n_rows & 3) == 0) A.flush(dx, dy, dz);
+        }
+        if ((ncn & 3) && tg == n_full) {
+            const uint4 e = R.next();
+            tmu_row<false>(S, e, ncn & 3, L, K, A);
+            tg += wpb;
+        }
+        sd = seg[++d];
+    }
+}
+
 }  // namespace tkhp

@@ -53,6 +53,10 @@ __host__ __device__ inline int atom_chunk_capacity(bool f64, int user_cap) {
 __host__ __device__ inline int atom_chunks_of(int count, int s_chunk) {
     return count < 1 ? 1 : (count + s_chunk - 1) / s_chunk;
 }
+// local index of the dummy record of a group: one past its largest chunk (<= s_chunk)
+__host__ __device__ inline int atom_dummy_index(int count, int n_chunks) {
+    return count < 1 ? 0 : (count + n_chunks - 1) / n_chunks;
+}
 
 // Rows of the far image the list builder keeps per warp (atom_lists.cu): 1.25 x the expected number
 // of neighbours of an atom in one chunk + 24, so that a chunk normally needs one segment (an

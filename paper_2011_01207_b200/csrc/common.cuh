@@ -26,6 +26,8 @@ struct DeviceState {
     int err_bad_alpha;      // alpha <= 0
     int err_bad_group;      // group id outside [0, N)
     int err_capacity;       // tile list or cluster list overflow
+    int err_barrier;        // a grid barrier of the persistent PCG kernel timed out
+    int pad_err;
     // grid (sort key)
     int grid_bits;          // b
     int pad0;
@@ -52,6 +54,8 @@ struct DeviceState {
     double pq, rr, gamma, delta;
     unsigned ticket;        // last-block reductions (reduce.cuh); 0 between kernels
     int bar_gen;            // grid barrier of k_pcg_step: the iteration whose partial sums are complete
+    unsigned bar_count;     // grid barrier of k_pcg_persist: arrivals (monotonic within a solve) ...
+    unsigned bar_release;   // ... and the last barrier every CTA has reached (adjacent: zeroed together)
     int conv_at;            // PCG: iterations with index >= conv_at are skipped on the device
     int iters;
 };
@@ -112,6 +116,9 @@ struct Ctx {
     double far_x0;          // a pair is FAR iff x = R^3 w_i w_j >= far_x0 and R >= far_rmin
     double far_rmin;
     float far_q[6];         // far fit of erfcx in t = 1/R
+    float4 *u32;            // n_pad: operand exchange of the persistent PCG kernel (atom_solve.cu)
+    bool coop_ok;           // the device supports cooperative launches
+    bool no_persist, no_fused_step;   // tkhp_params.solver_flags
     bool fuse_q;            // ATOM-mode T.mu kernel also forms q = p/alpha - T p - self p and p.q (PCG)
     int spec_iter;          // >= 0: the pair kernel about to be launched belongs to PCG iteration spec_iter
     DeviceState *h_state;   // pinned host copy of *st (list header), valid when header_valid
@@ -130,10 +137,11 @@ struct Ctx {
     // launch accounting / live kernel timing (tkhp_profile_*)
     long long n_launches;               // kernels launched since the last reset
     bool prof;                          // record an event pair around every T.mu / field pair kernel
-    int prof_n[2];                      // [0] T.mu launches, [1] field launches recorded
-    cudaEvent_t prof_ev[2][2 * 64];
-    int prof_iter[2][64];               // PCG iteration the recorded launch belongs to (-1: unconditional)
-    bool prof_skip[2][64];              // the launch was a speculative no-op (iteration after convergence)
+    int prof_n[3];                      // [0] T.mu launches, [1] field launches, [2] persistent solve kernels recorded
+    cudaEvent_t prof_ev[3][2 * 64];
+    int prof_iter[3][64];               // PCG iteration the recorded launch belongs to (-1: unconditional)
+    bool prof_skip[3][64];              // the launch was a speculative no-op (iteration after convergence)
+    long long prof_solve_matvecs;       // T.mu products done inside the recorded persistent solve kernels
     long long n_noop_launches;          // launches that returned at once for the same reason
 };
 constexpr int PROF_MAX = 64;
@@ -187,6 +195,9 @@ void atom_far_setup(Ctx *c);
 int atom_lists_configure(Ctx *c);
 int atom_pairs_configure(Ctx *c);
 int cluster_pairs_configure(Ctx *c);
+int atom_solve_configure(Ctx *c);
+bool atom_solve_eligible(Ctx *c);
+int atom_solve_launch(Ctx *c, double tol, int max_iter, cudaStream_t s);
 int atom_tmatvec(Ctx *c, cudaStream_t s);
 int atom_field(Ctx *c, cudaStream_t s);
 long long atom_slots(Ctx *c);

@@ -434,9 +434,40 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
         int per_sm = 0;
         const void *fn = mixed ? (const void *)k_pcg_step<float4> : (const void *)k_pcg_step<double4>;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, VEC_THREADS, 0) == cudaSuccess)
-            fused_step = g1 <= per_sm * c->sm_count && g1 <= c->part_cap;
+            fused_step = c->coop_ok && !c->no_fused_step && g1 <= per_sm * c->sm_count && g1 <= c->part_cap;
         else
             cudaGetLastError();
+    }
+
+    // ---- the whole solve as one persistent cooperative kernel (atom_solve.cu) when it can run
+    if (atom_solve_eligible(c)) {
+        k_pcg_init<float4><<<g1, VEC_THREADS, 0, s>>>(d_field, d_mu, use_guess, c->perm, c->alpha_s, n_pad, c->vE, c->vmu, c->mu32, c->st);
+        c->n_launches += 1;
+        const bool rec = c->prof && c->prof_n[2] < PROF_MAX;
+        if (rec) cudaEventRecord(c->prof_ev[2][2 * c->prof_n[2]], s);
+        rc = atom_solve_launch(c, tol, max_iter, s);
+        if (rec) { cudaEventRecord(c->prof_ev[2][2 * c->prof_n[2] + 1], s); c->prof_n[2]++; }
+        if (rc) {
+            cudaStreamSynchronize(s);
+            return rc;
+        }
+        k_unsort3<<<g1, VEC_THREADS, 0, s>>>(c->vmu, c->perm, n_pad, d_mu);
+        c->n_launches += 1;
+        TKHP_CUDA(c, cudaGetLastError());
+        TKHP_CUDA(c, cudaMemcpyAsync(c->h_scalars, &c->st->rr, sizeof(double), cudaMemcpyDeviceToHost, s));
+        TKHP_CUDA(c, cudaMemcpyAsync(c->h_scalars + 1, &c->st->iters, sizeof(int), cudaMemcpyDeviceToHost, s));
+        TKHP_CUDA(c, cudaMemcpyAsync(c->h_scalars + 2, &c->st->err_barrier, sizeof(int), cudaMemcpyDeviceToHost, s));
+        TKHP_CUDA(c, cudaStreamSynchronize(s));
+        int it_done, bar_err;
+        memcpy(&it_done, c->h_scalars + 1, sizeof(int));
+        memcpy(&bar_err, c->h_scalars + 2, sizeof(int));
+        if (bar_err) return set_err(c, TKHP_ECUDA, "grid barrier of the persistent PCG kernel timed out%s");
+        if (rec) c->prof_solve_matvecs += it_done + 1;
+        const double rms_done = sqrt(c->h_scalars[0] / c->n);
+        if (h_iters) *h_iters = it_done;
+        if (h_rms) *h_rms = rms_done;
+        if (!(rms_done < tol)) return set_err(c, TKHP_ENOCONV, "PCG did not reach the tolerance within max_iter%s");
+        return TKHP_OK;
     }
 
     for (int k = 0; k < RING; ++k) c->h_ring[k] = -1.0;

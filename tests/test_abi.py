@@ -49,7 +49,7 @@ def test_params_struct_layout_matches_header(built_lib, tmp_path):
     subprocess.run(["gcc", "-I", str(ROOT / "include"), str(src), "-o", str(exe)], check=True)
     out = dict(line.split() for line in subprocess.run([str(exe)], check=True, capture_output=True,
                                                        text=True).stdout.splitlines())
-    assert int(out["sizeof"]) == ctypes.sizeof(pk.TkhpParams) == 72
+    assert int(out["sizeof"]) == ctypes.sizeof(pk.TkhpParams) == 80
     for n in names:
         assert int(out[n]) == getattr(pk.TkhpParams, n).offset, n
 
