@@ -213,7 +213,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     d_field = torch.empty((n, 3), dtype=f64, device=dev)
     d_mu = torch.empty((n, 3), dtype=f64, device=dev)
     d_energy = torch.empty((), dtype=f64, device=dev)
-    stream = torch.cuda.current_stream()
+    torch.cuda.synchronize()
+    # a stream of our own (the library replays its list build as a CUDA graph, which the legacy default
+    # stream cannot capture); it is made torch's current stream, so the events below see it
+    stream = torch.cuda.Stream(device=dev)
+    torch.cuda.set_stream(stream)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def step():

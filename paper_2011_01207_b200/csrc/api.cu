@@ -241,6 +241,7 @@ int tkhp_destroy(tkhp_ctx *ctx) {
     cudaStreamDestroy(c->copy_stream);
     for (int w = 0; w < 3; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventDestroy(c->prof_ev[w][i]);
+    if (c->build_graph) cudaGraphExecDestroy(c->build_graph);
     cudaFreeHost(c->h_ring);
     cudaFreeHost(c->h_scalars);
     cudaFreeHost(c->h_state);
@@ -253,17 +254,11 @@ const char *tkhp_last_error(const tkhp_ctx *ctx) {
     return reinterpret_cast<const Ctx *>(ctx)->err;
 }
 
-int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polarizability,
-                      const int32_t *d_group_id, void *stream) {
-    if (!ctx) return TKHP_EINVAL;
-    Ctx *c = reinterpret_cast<Ctx *>(ctx);
-    if (!d_pos || !d_polarizability || !d_group_id) return set_err(c, TKHP_EINVAL, "NULL input%s");
-    cudaStream_t s = static_cast<cudaStream_t>(stream);
-    tic(c, 0, s);
+// everything tkhp_nblist_build enqueues: the prescribed block-pair list, then the finer lists
+static int enqueue_build(Ctx *c, const double *d_pos, const double *d_polarizability, const int32_t *d_group_id,
+                         cudaStream_t s) {
     int rc = nblist_build(c, d_pos, d_polarizability, d_group_id, s);
     if (rc) return rc;
-    c->built = true;
-    c->list_mode_in_use = TKHP_LIST_TILES;
     if (c->p.list_mode != TKHP_LIST_TILES) {
         rc = cluster_build(c, s);
         if (rc) return rc;
@@ -272,6 +267,53 @@ int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polari
             if (rc) return rc;
         }
     }
+    return TKHP_OK;
+}
+
+int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polarizability,
+                      const int32_t *d_group_id, void *stream) {
+    if (!ctx) return TKHP_EINVAL;
+    Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    if (!d_pos || !d_polarizability || !d_group_id) return set_err(c, TKHP_EINVAL, "NULL input%s");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    tic(c, 0, s);
+    c->header_valid = false;
+    int rc = TKHP_OK;
+    const bool same = c->build_graph && c->build_key[0] == d_pos && c->build_key[1] == d_polarizability &&
+                      c->build_key[2] == d_group_id;
+    if (!same && !c->no_graph && s != nullptr) {
+        // capture the build once for these pointers (the legacy default stream cannot be captured)
+        if (c->build_graph) { cudaGraphExecDestroy(c->build_graph); c->build_graph = nullptr; }
+        cudaGraph_t graph = nullptr;
+        const long long before = c->n_launches;
+        if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            rc = enqueue_build(c, d_pos, d_polarizability, d_group_id, s);
+            const cudaError_t e = cudaStreamEndCapture(s, &graph);
+            if (rc == TKHP_OK && e == cudaSuccess && graph &&
+                cudaGraphInstantiate(&c->build_graph, graph, 0) == cudaSuccess) {
+                c->build_key[0] = d_pos; c->build_key[1] = d_polarizability; c->build_key[2] = d_group_id;
+                c->build_graph_launches = c->n_launches - before;
+            } else {
+                c->build_graph = nullptr;
+                c->no_graph = true;
+                rc = TKHP_OK;
+            }
+            if (graph) cudaGraphDestroy(graph);
+            c->n_launches = before;
+        } else {
+            c->no_graph = true;
+        }
+        cudaGetLastError();
+    }
+    if (c->build_graph && c->build_key[0] == d_pos && c->build_key[1] == d_polarizability && c->build_key[2] == d_group_id) {
+        TKHP_CUDA(c, cudaGraphLaunch(c->build_graph, s));
+        c->n_launches += c->build_graph_launches;
+    } else {
+        rc = enqueue_build(c, d_pos, d_polarizability, d_group_id, s);
+        if (rc) return rc;
+    }
+    c->built = true;
+    c->list_mode_in_use = TKHP_LIST_TILES;
     toc(c, 0, s);
     return TKHP_OK;
 }

@@ -7,12 +7,15 @@
 // R^2 <= r_c^2 for the positions of the build, so the pair kernels contain no cutoff test.  The
 // candidates of an atom are the entries of its 8-atom cluster's list (cluster_build.cu).
 //
-// One CTA per group, one warp per block, one lane per atom; chunk by chunk the staged positions
-// are put in shared memory and every lane walks its cluster's list.  A hit is classified
+// Pass 1 (k_atom_scan): one CTA per group, one warp per block, one lane per atom; chunk by chunk the
+// staged positions are put in shared memory and every lane walks its cluster's list.  A hit is classified
 //   FAR   x = R^3 w_i w_j >= x0 (e^-x below FP32 resolution: the Thole term is dropped) and
 //         R >= R_far (z = beta R inside the range of the far-field erfcx fit), or
 //   NEAR  otherwise (full formula),
-// and dealt straight into its final position of a per-warp shared-memory IMAGE of the segment:
+// and appended to its class of the open segment.  Pass 2 (k_atom_deal, one warp per block) then puts
+// every class of every segment into its final order through a per-warp shared-memory IMAGE (the
+// image is 16 KB per warp: inside pass 1 it would leave room for 7 warps per SM, and that pass is
+// latency bound):
 // the pair kernels gather a 16-byte and an 8-byte record from shared memory, one per lane and step;
 // a quarter warp's LDS.128 (a half warp's LDS.64) is served in one wavefront only if its 8 (16)
 // records have different indices mod 8 (mod 16).  Lane l therefore keeps 16 columns per class,
@@ -25,27 +28,29 @@
 
 namespace tkhp {
 
-// one class (far or near) of one lane's image: 16 column counters of 8 bits
+// One class (far or near) of one lane's image.  The 16 column counters of a lane are bytes in shared
+// memory, cnt[column * 32] (a register array indexed per lane would cost a dozen instructions per
+// access): k_atom_lists is bound by its instruction count.
 struct Deal {
-    unsigned long long c0 = 0ull, c1 = 0ull;
+    uint8_t *cnt;      // this lane's counters: cnt[b * 32], b = 0..15
     int k = 0;
-    __device__ __forceinline__ unsigned get(unsigned b) const { return (unsigned)(((b & 8u) ? c1 : c0) >> (8 * (b & 7u))) & 0xffu; }
-    __device__ __forceinline__ void inc(unsigned b) {
-        const unsigned long long one = 1ull << (8 * (b & 7u));
-        if (b & 8u) c1 += one; else c0 += one;
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int b = 0; b < 16; ++b) cnt[b * 32] = 0;
+        k = 0;
     }
 };
 
 // put one entry into the image; a full column spills into the next one (only a bank conflict later)
 __device__ __forceinline__ void deal(Deal &d, uint16_t *img, int colcap, unsigned l16, unsigned off, unsigned bank) {
-    unsigned b = bank, r = d.get(b);
+    unsigned b = bank, r = d.cnt[b * 32];
     while (r >= (unsigned)colcap) {
         b = (b + 1) & 15u;
-        r = d.get(b);
+        r = d.cnt[b * 32];
     }
     const unsigned t = ((b - l16) & 15u) + 16u * r;
     img[t * 32] = (uint16_t)off;
-    d.inc(b);
+    d.cnt[b * 32] = (uint8_t)(r + 1);
     ++d.k;
 }
 
@@ -54,15 +59,15 @@ __device__ __forceinline__ unsigned col_cap(unsigned j, unsigned len) { return j
 
 // entries of over-full columns -> holes of under-full ones (per lane, no cross-lane traffic)
 __device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16, unsigned len) {
-    unsigned hb = 0, hr = d.get(0);
+    unsigned hb = 0, hr = d.cnt[0];
     for (unsigned b = 0; b < 16; ++b) {
         const unsigned j = (b - l16) & 15u;
-        const unsigned cb = d.get(b);
+        const unsigned cb = d.cnt[b * 32];
         for (unsigned r = col_cap(j, len); r < cb; ++r) {
             const uint16_t v = img[(j + 16u * r) * 32];
             while (hr >= col_cap((hb - l16) & 15u, len)) {
                 ++hb;
-                hr = d.get(hb);
+                hr = d.cnt[hb * 32];
             }
             img[(((hb - l16) & 15u) + 16u * hr) * 32] = v;
             ++hr;
@@ -70,14 +75,17 @@ __device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16
     }
 }
 
+// ---- pass 1: scan.  One CTA per group, one warp per block, one lane per atom.  FAR hits go straight
+// to the block's rows in arrival order (pass 2 permutes them in place), NEAR hits wait in a small
+// shared-memory buffer until the length of the far part of the segment is known.
 template <typename real>
 __global__ void __launch_bounds__(GT)
-k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
-             const typename Vec4<real>::type *__restrict__ stage_pos, real rc2, real far_x2, real far_r2,
-             int s_chunk, DeviceState *st) {
+k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
+            const typename Vec4<real>::type *__restrict__ stage_pos, real rc2, real far_x2, real far_r2,
+            int s_chunk, DeviceState *st) {
     using vec4 = typename Vec4<real>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);
+    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk] | near buffers [GB][NEAR_CAP][32] u16
 
     const int g = blockIdx.x, t = threadIdx.x, lane = t & 31, w = t >> 5;
     const int b0 = ws.group_first[g], nb = ws.group_first[g + 1] - b0;
@@ -87,9 +95,12 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const bool active = w < nb;
     const int blk = b0 + (active ? w : 0);
     int2 *__restrict__ seg = ws.aseg + (size_t)blk * NSEG_MAX;
+    // padding entries point at the record after the largest chunk of THIS group (the kernels put a
+    // far-away record with zero payload there)
+    const unsigned dummy = (unsigned)atom_dummy_index(count, n_chunks) * (unsigned)sizeof(vec4);
     if (n_chunks > NCH_MAX) {                      // uniform over the CTA
         if (t == 0) st->atom_bad = 1;
-        if (active && lane == 0) seg[0] = seg[NSEG_MAX - 1] = make_int2((int)(0xffu << 24), 0);
+        if (active && lane == 0) seg[0] = seg[NSEG_MAX - 1] = make_int2((int)(0xffu << 24), (int)dummy);
         return;
     }
     const unsigned magic = ((1u << 20) + (unsigned)n_chunks - 1u) / (unsigned)n_chunks;   // e / n for e < 2^16
@@ -99,27 +110,27 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int L = active ? ws.oct_len[oct] : 0;
     const uint4 *__restrict__ ent8 = reinterpret_cast<const uint4 *>(ws.entries + (size_t)oct * ws.l_cap);  // 8 entries per load
     const int L8 = L >> 3;                                                                                   // L is a multiple of 8
-    uint4 *__restrict__ rows = reinterpret_cast<uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;    // row r of this lane: rows[r * 32]
+    // row r of this lane as two quads of 4 entries: quads[2 * (r * 32) + h]
+    uint2 *__restrict__ quads = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + 2 * lane;
     const int rows_cap = ws.a_cap >> 3;
-    // padding entries point at the record after the largest chunk of THIS group (the kernels put a
-    // far-away record with zero payload there)
-    const unsigned dummy = (unsigned)atom_dummy_index(count, n_chunks) * (unsigned)sizeof(vec4);
-    const unsigned l16 = (unsigned)lane & 15u;
-    const int fcap = ws.far_cap, fcol = fcap >> 4, ncol = NEAR_CAP >> 4;
-    uint16_t *img_f = reinterpret_cast<uint16_t *>(smem_raw + (size_t)s_chunk * sizeof(vec4)) +
-                      (size_t)(active ? w : 0) * (fcap + NEAR_CAP) * 32 + lane;          // img[row * 32]
-    uint16_t *img_n = img_f + (size_t)fcap * 32;
+    const unsigned long long dummy4 = 0x0001000100010001ull * (unsigned long long)dummy;
+    const int fcap = ws.far_cap;
+    uint16_t *nbuf = reinterpret_cast<uint16_t *>(smem_raw + (size_t)s_chunk * sizeof(vec4)) +
+                     (size_t)w * NEAR_CAP * 32 + lane;                                   // nbuf[k * 32]
 
     int row_cur = 0, nseg = 0;
     long long slots = 0, slots_far = 0;
     bool bad = false;
-    Deal F, N;
-    if (active)
-        for (int r = 0; r < fcap + NEAR_CAP; ++r) img_f[r * 32] = 0xffffu;
+    int kf = 0, kn = 0;                  // far / near entries of this lane in the open segment
+    unsigned long long pend = 0;         // the far quad being filled
 
-    // pads, levels and writes out the segment collected so far (warp-uniform control flow)
-    auto flush = [&](int c) {
-        int fmax = F.k, nmax = N.k;
+    auto put_quad = [&](int q, unsigned long long v) {      // quad q of the open segment's far part
+        const int r = row_cur + (q >> 1);
+        if (r < rows_cap) quads[(size_t)r * 64 + (q & 1)] = make_uint2((unsigned)v, (unsigned)(v >> 32));
+    };
+    // closes the open segment: pads both classes to the longest lane, writes the near rows and the descriptor
+    auto close_segment = [&](int c) {
+        int fmax = kf, nmax = kn;
         for (int o = 16; o > 0; o >>= 1) {
             fmax = max(fmax, __shfl_xor_sync(0xffffffffu, fmax, o));
             nmax = max(nmax, __shfl_xor_sync(0xffffffffu, nmax, o));
@@ -130,26 +141,15 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         if (row_cur + fr + nr > rows_cap || nseg >= NSEG_MAX - 1) {
             bad = true;                                                       // capacity: CLUSTER lists are used
         } else {
-            level(F, img_f, l16, 2u * ncf);
-            level(N, img_n, l16, 2u * ncn);
-            for (int part = 0; part < 2; ++part) {
-                uint16_t *img = part ? img_n : img_f;
-                const int nrow = part ? nr : fr, len = 2 * (part ? ncn : ncf);
-                uint4 *out = rows + (size_t)(row_cur + (part ? fr : 0)) * 32;
-                for (int q = 0; q < nrow; ++q, out += 32) {
-                    unsigned v[8];
+            int q = kf >> 2;                                                  // first far quad not stored yet
+            if (kf & 3) { put_quad(q, pend | (dummy4 << ((kf & 3) * 16))); ++q; }
+            for (; q < 2 * fr; ++q) put_quad(q, dummy4);
+            uint4 *out = reinterpret_cast<uint4 *>(quads) + (size_t)(row_cur + fr) * 32;
+            for (int r = 0; r < nr; ++r, out += 32) {
+                unsigned v[8];
 #pragma unroll
-                    for (int h = 0; h < 8; ++h) {
-                        const int e = 8 * q + h;
-                        const unsigned x = img[e * 32];
-                        v[h] = (e >= len || x == 0xffffu) ? dummy : x;
-                        img[e * 32] = 0xffffu;
-                    }
-                    *out = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
-                }
-                // rows of the image beyond the written ones that the spill of a full column touched
-                const int used = part ? NEAR_CAP : fcap;
-                for (int e = 8 * nrow; e < used; ++e) img[e * 32] = 0xffffu;
+                for (int h = 0; h < 8; ++h) v[h] = 8 * r + h < kn ? nbuf[(8 * r + h) * 32] : dummy;
+                *out = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
             }
             if (lane == 0) seg[nseg] = make_int2(row_cur | (c << 24), ncf | (ncn << 16));
             ++nseg;
@@ -157,8 +157,7 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             slots += 2 * (ncf + ncn);
             slots_far += 2 * ncf;
         }
-        F = Deal();
-        N = Deal();
+        kf = 0; kn = 0; pend = 0;
     };
 
     for (int c = 0; c < n_chunks; ++c) {
@@ -174,7 +173,7 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             if (v + 1 < L8) nxt = ent8[v + 1];           // one address per quarter warp, one load ahead
             const unsigned word[4] = {cur.x, cur.y, cur.z, cur.w};
             // the 8 entries of the vector are tested together (8 independent chains), then the hits
-            // are dealt in list order
+            // are appended in list order
             unsigned loc[8];
             bool hit[8], far[8];
 #pragma unroll
@@ -197,17 +196,24 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             for (int h = 0; h < 8; ++h) {
                 if (hit[h]) {
                     const unsigned off = loc[h] * (unsigned)sizeof(vec4);
-                    if (far[h]) deal(F, img_f, fcol, l16, off, loc[h] & 15u);
-                    else deal(N, img_n, ncol, l16, off, loc[h] & 15u);
+                    if (far[h]) {
+                        pend |= (unsigned long long)off << ((kf & 3) * 16);
+                        if ((kf & 3) == 3) { put_quad(kf >> 2, pend); pend = 0; }
+                        ++kf;
+                    } else {
+                        nbuf[kn * 32] = (uint16_t)off;
+                        ++kn;
+                    }
                 }
             }
-            // a vector adds at most 8 entries to a class: start another segment before one overflows
-            if (__any_sync(0xffffffffu, F.k > fcap - 8 || N.k > NEAR_CAP - 8)) flush(c);
+            // a vector adds at most 8 entries to a class: close the segment before pass 2's image or the
+            // near buffer could overflow
+            if (__any_sync(0xffffffffu, kf > fcap - 8 || kn > NEAR_CAP - 8)) close_segment(c);
         }
-        flush(c);
+        close_segment(c);
     }
     if (active && lane == 0) {
-        seg[nseg] = seg[NSEG_MAX - 1] = make_int2(row_cur | (int)(0xffu << 24), 0);    // terminator; total rows also in the last slot
+        seg[nseg] = seg[NSEG_MAX - 1] = make_int2(row_cur | (int)(0xffu << 24), (int)dummy);    // terminator (y = the dummy offset); total rows also in the last slot
         if (bad) st->atom_bad = 1;
         atomicAdd((unsigned long long *)&st->n_atom_entries, (unsigned long long)slots);
         atomicAdd((unsigned long long *)&st->n_atom_far, (unsigned long long)slots_far);
@@ -215,36 +221,98 @@ k_atom_lists(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     }
 }
 
+// ---- pass 2: deal.  One warp per block: every class of every segment is read into the image in the
+// bank-aware layout (header comment), levelled, and written back in place.
+constexpr int DEAL_WARPS = 4;
+
+__global__ void __launch_bounds__(DEAL_WARPS * 32)
+k_atom_deal(ClusterWs ws, int n_blocks) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int blk = blockIdx.x * DEAL_WARPS + w;
+    if (blk >= n_blocks) return;
+    const int fcap = ws.far_cap;
+    const int img_rows = fcap > NEAR_CAP ? fcap : NEAR_CAP;
+    uint16_t *img = reinterpret_cast<uint16_t *>(smem_raw) + (size_t)w * img_rows * 32 + lane;       // img[row * 32]
+    Deal D;
+    D.cnt = smem_raw + (size_t)DEAL_WARPS * img_rows * 32 * sizeof(uint16_t) + (size_t)w * 512 + lane;
+    const unsigned l16 = (unsigned)lane & 15u;
+    uint4 *__restrict__ rows = reinterpret_cast<uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
+    const int2 *__restrict__ seg = ws.aseg + (size_t)blk * NSEG_MAX;
+    const unsigned dummy = (unsigned)seg[NSEG_MAX - 1].y;
+    for (int r = 0; r < img_rows; ++r) img[r * 32] = 0xffffu;
+    D.clear();
+
+    for (int d = 0; d < NSEG_MAX; ++d) {
+        const int2 sd = seg[d];
+        if (seg_chunk(sd) == 0xff) break;
+        const int nc[2] = {seg_far_calls(sd), seg_near_calls(sd)};
+        int r0 = seg_row0(sd);
+        for (int cls = 0; cls < 2; ++cls) {
+            const int nrow = (nc[cls] + 3) >> 2, len = 2 * nc[cls];
+            uint4 *p = rows + (size_t)r0 * 32;
+            r0 += nrow;
+            if (nrow == 0 || 8 * nrow > img_rows) continue;          // (an over-long class keeps its arrival order)
+            const int colcap = (8 * nrow + 15) >> 4;
+            uint4 nxt = p[0];
+            for (int q = 0; q < nrow; ++q) {
+                const uint4 e = nxt;
+                if (q + 1 < nrow) nxt = p[(size_t)(q + 1) * 32];
+                const unsigned v[8] = {e.x & 0xffffu, e.x >> 16, e.y & 0xffffu, e.y >> 16,
+                                       e.z & 0xffffu, e.z >> 16, e.w & 0xffffu, e.w >> 16};
+#pragma unroll
+                for (int h = 0; h < 8; ++h)
+                    if (v[h] != dummy) deal(D, img, colcap, l16, v[h], (v[h] >> 4) & 15u);
+            }
+            level(D, img, l16, (unsigned)len);
+            for (int q = 0; q < nrow; ++q) {
+                unsigned v[8];
+#pragma unroll
+                for (int h = 0; h < 8; ++h) {
+                    const int e = 8 * q + h;
+                    const unsigned x = img[e * 32];
+                    v[h] = (e >= len || x == 0xffffu) ? dummy : x;
+                    img[e * 32] = 0xffffu;
+                }
+                p[(size_t)q * 32] = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
+            }
+            // cells beyond the written rows that the spill of a full column touched
+            for (int e = 8 * nrow; e < 16 * colcap && e < img_rows; ++e) img[e * 32] = 0xffffu;
+            D.clear();
+        }
+    }
+}
+
 // ----------------------------------------------------------------------------- host side
-size_t atom_lists_smem(const ClusterWs &ws, bool f64, int nb_max) {
-    const int s_chunk = atom_chunk_capacity(f64, ws.chunk_cap);
-    return (size_t)s_chunk * (f64 ? sizeof(double4) : sizeof(float4)) +
-           (size_t)nb_max * (ws.far_cap + NEAR_CAP) * 32 * sizeof(uint16_t);
+static size_t deal_smem(const ClusterWs &ws) {
+    const int img_rows = ws.far_cap > NEAR_CAP ? ws.far_cap : NEAR_CAP;
+    return (size_t)DEAL_WARPS * ((size_t)img_rows * 32 * sizeof(uint16_t) + 512);
 }
 
 int atom_build(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
     const bool f64 = c->p.precision == TKHP_FP64;
     const int s_chunk = atom_chunk_capacity(f64, ws.chunk_cap);
-    const int nb_max = (c->n_blocks + ws.n_groups - 1) / ws.n_groups;
-    const size_t smem = atom_lists_smem(ws, f64, nb_max);
+    const size_t smem = (size_t)s_chunk * (f64 ? sizeof(double4) : sizeof(float4)) + (size_t)GB * NEAR_CAP * 32 * sizeof(uint16_t);
     const double rc2 = c->p.cutoff * c->p.cutoff;
     // far class off (FP64, beta = 0): far_r2 < 0 puts every pair into the first class of rows, which
     // the kernels then evaluate with the full formula
     const double x2 = c->far_on ? c->far_x0 * c->far_x0 : 0.0, r2_far = c->far_on ? c->far_rmin * c->far_rmin : -1.0;
     if (f64)
-        k_atom_lists<double><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos64, ws.stage_pos64, rc2, x2, r2_far, s_chunk, c->st);
+        k_atom_scan<double><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos64, ws.stage_pos64, rc2, x2, r2_far, s_chunk, c->st);
     else
-        k_atom_lists<float><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos32, ws.stage_pos32, (float)rc2, (float)x2,
-                                                           (float)r2_far, s_chunk, c->st);
-    c->n_launches += 1;
+        k_atom_scan<float><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos32, ws.stage_pos32, (float)rc2, (float)x2,
+                                                          (float)r2_far, s_chunk, c->st);
+    k_atom_deal<<<div_up(c->n_blocks, DEAL_WARPS), DEAL_WARPS * 32, deal_smem(ws), s>>>(ws, c->n_blocks);
+    c->n_launches += 2;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }
 
 int atom_lists_configure(Ctx *c) {
-    TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_lists<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_lists<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_scan<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_scan<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_deal, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
     return TKHP_OK;
 }
 

@@ -104,30 +104,56 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
         for (int k = 0; k < 3; ++k) { s_olo[t][k] = lo[k]; s_ohi[t][k] = hi[k]; }
     }
 
-    // (d) candidate blocks: warp 0 walks super-blocks, then blocks, in index order (deterministic)
-    if (w == 0) {
+    // (d) candidate blocks: in every round of 256 super-blocks warp w takes 32 consecutive ones (one
+    // per lane), then the blocks of its hits; the warps' hits are concatenated in warp order, i.e.
+    // in block index order (deterministic).
+    {
         const double reach2 = rcm * rcm;
-        int n = 0;
-        for (int s0 = 0; s0 < n_super; s0 += 32) {
-            const int sj = s0 + lane;
+        int n = 0;                                   // candidates found so far (uniform over the CTA)
+        for (int s0 = 0; s0 < n_super; s0 += GB * 32) {
+            // one super-block per lane: 32 consecutive super-blocks per warp
+            const int sj = s0 + w * 32 + lane;
             bool cand = false;
             if (sj < n_super) cand = gap2_boxes(s_gc, s_gh, scentre[sj], shalf[sj], box) <= reach2;
             unsigned m = __ballot_sync(0xffffffffu, cand);
-            while (m) {
-                const int s = s0 + (__ffs(m) - 1);
-                m &= m - 1;
-                const int J = s * SUPER + lane;
+            // two passes over the warp's candidate super-blocks: count, then write at the warp's offset
+            int mine = 0;
+            unsigned mm = m;
+            while (mm) {
+                const int sb = s0 + w * 32 + (__ffs(mm) - 1);
+                mm &= mm - 1;
+                const int J = sb * SUPER + lane;
+                bool keep = false;
+                if (J < n_blocks) keep = gap2_boxes(s_gc, s_gh, bcentre[J], bhalf[J], box) <= reach2;
+                mine += __popc(__ballot_sync(0xffffffffu, keep));
+            }
+            if (lane == 0) s_wsum[w] = mine;
+            __syncthreads();
+            int before = 0, total = 0;
+            for (int k = 0; k < GB; ++k) {
+                const int v = s_wsum[k];
+                if (k < w) before += v;
+                total += v;
+            }
+            int pos0 = n + before;
+            mm = m;
+            while (mm) {
+                const int sb = s0 + w * 32 + (__ffs(mm) - 1);
+                mm &= mm - 1;
+                const int J = sb * SUPER + lane;
                 bool keep = false;
                 if (J < n_blocks) keep = gap2_boxes(s_gc, s_gh, bcentre[J], bhalf[J], box) <= reach2;
                 const unsigned km = __ballot_sync(0xffffffffu, keep);
                 if (keep) {
-                    const int pos = n + __popc(km & ((1u << lane) - 1u));
+                    const int pos = pos0 + __popc(km & ((1u << lane) - 1u));
                     if (pos < CB_CAP) s_cand[pos] = J;
                 }
-                n += __popc(km);
+                pos0 += __popc(km);
             }
+            n += total;
+            __syncthreads();
         }
-        if (lane == 0) {
+        if (t == 0) {
             if (n > CB_CAP) { st->cluster_bad = 1; n = CB_CAP; }
             s_ncand = n;
         }
@@ -161,20 +187,27 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
                     px -= box * rint(px / box); py -= box * rint(py / box); pz -= box * rint(pz / box);
                 }
                 pj = make_float4((float)px, (float)py, (float)pz, p.w);
+                // first the 32 cluster boxes (uniform loop), then the atoms of the clusters whose box
+                // is within reach (a loop over the set bits: ~1/4 of the clusters)
+                uint32_t near_box = 0;
+#pragma unroll 8
                 for (int o = 0; o < OCT; ++o) {
                     const float ex = fmaxf(0.f, fmaxf(s_olo[o][0] - pj.x, pj.x - s_ohi[o][0]));
                     const float ey = fmaxf(0.f, fmaxf(s_olo[o][1] - pj.y, pj.y - s_ohi[o][1]));
                     const float ez = fmaxf(0.f, fmaxf(s_olo[o][2] - pj.z, pj.z - s_ohi[o][2]));
-                    if (ex * ex + ey * ey + ez * ez <= rcm2) {
-                        bool any = false;
+                    if (ex * ex + ey * ey + ez * ez <= rcm2) near_box |= 1u << o;
+                }
+                while (near_box) {
+                    const int o = __ffs(near_box) - 1;
+                    near_box &= near_box - 1;
+                    bool any = false;
 #pragma unroll
-                        for (int a = 0; a < CLUSTER; ++a) {
-                            const float4 q = s_i[o * CLUSTER + a];
-                            const float ddx = q.x - pj.x, ddy = q.y - pj.y, ddz = q.z - pj.z;
-                            any |= (ddx * ddx + ddy * ddy + ddz * ddz <= rcm2) && (q.w > 0.f);
-                        }
-                        if (any) mask |= 1u << o;
+                    for (int a = 0; a < CLUSTER; ++a) {
+                        const float4 q = s_i[o * CLUSTER + a];
+                        const float ddx = q.x - pj.x, ddy = q.y - pj.y, ddz = q.z - pj.z;
+                        any |= (ddx * ddx + ddy * ddy + ddz * ddz <= rcm2) && (q.w > 0.f);
                     }
+                    if (any) mask |= 1u << o;
                 }
             }
         }

@@ -132,6 +132,13 @@ struct Ctx {
     void *cl_ws;
     size_t cl_ws_bytes;
 
+    // CUDA graph of one whole list build (about 30 small kernels, memsets and copies: launch bound),
+    // re-used while the caller passes the same input pointers
+    cudaGraphExec_t build_graph;
+    const void *build_key[3];           // d_pos, d_polarizability, d_group_id the graph was captured with
+    long long build_graph_launches;     // kernels inside the graph
+    bool no_graph;                      // capture failed once: plain launches from then on
+
     cudaEvent_t ev[10];
     double last_ms[5];
     // launch accounting / live kernel timing (tkhp_profile_*)
