@@ -284,11 +284,15 @@ def grid_bits(extent: float) -> int:
     return b
 
 
+OPEN_MAX_BITS = 6     # DESIGN.md "Sort key" (Q14): an open-boundary grid has at most 2^6 cells per axis
+
+
 def cell_coords(pos: np.ndarray, box: float):
     """integer cell coordinates on a 2^b grid.
 
     periodic: w = wrap(x), extent = L, origin 0.  open boundary: origin = per-axis
-    minimum, extent = 1.000001 * max_axis(max - min) + 1e-9.
+    minimum, extent = 1.000001 * max_axis(max - min) + 1e-9, b <= 6 (wider systems get
+    coarser cells: the order stays a deterministic function of the coordinates).
     cell = min(2^b - 1, floor(w * inv_h)), inv_h = 2^b / extent.
     Returns (cells (N,3) int64, b).
     """
@@ -301,6 +305,8 @@ def cell_coords(pos: np.ndarray, box: float):
         w = pos - lo[None, :]
         extent = float((pos.max(axis=0) - lo).max()) * 1.000001 + 1e-9
     b = grid_bits(extent)
+    if box <= 0:
+        b = min(b, OPEN_MAX_BITS)
     inv_h = float(1 << b) / extent
     cells = np.floor(w * inv_h).astype(np.int64)
     cells = np.minimum(cells, (1 << b) - 1)

@@ -289,6 +289,10 @@ class Polarizer:
         except Exception:
             pass
 
+    def _s(self, stream):
+        """The caller's stream, else the current stream of THIS context's device."""
+        return self.torch.cuda.current_stream(self.device) if stream is None else stream
+
     def _f64(self, a):
         return self.torch.as_tensor(a, dtype=self.torch.float64, device=self.device).contiguous()
 
@@ -298,12 +302,12 @@ class Polarizer:
         self._pos = self._f64(pos)
         self._alpha = self._f64(polarizability)
         self._group = t.as_tensor(group_id, dtype=t.int32, device=self.device).contiguous()
-        tkhp_nblist_build(self.ctx, self._pos, self._alpha, self._group, stream)
+        tkhp_nblist_build(self.ctx, self._pos, self._alpha, self._group, self._s(stream))
 
     def nblist_view(self, stream=None):
         """-> (perm (32*n_blocks,) int32 CPU numpy, pairs (T,2) int32 CPU numpy)."""
         import numpy as np
-        nb, npairs, p_perm, p_pairs = tkhp_nblist_view(self.ctx, stream)
+        nb, npairs, p_perm, p_pairs = tkhp_nblist_view(self.ctx, self._s(stream))
         off_perm = p_perm - self._ws_ptr
         off_pairs = p_pairs - self._ws_ptr
         base = self._ws_ptr - self.workspace.data_ptr()
@@ -313,23 +317,23 @@ class Polarizer:
         return perm.cpu().numpy().copy(), pairs.cpu().numpy().reshape(-1, 2).copy()
 
     def nblist_stats(self, stream=None, count_pairs=True):
-        return tkhp_nblist_stats(self.ctx, stream, count_pairs)
+        return tkhp_nblist_stats(self.ctx, self._s(stream), count_pairs)
 
     def nblist_atom_stats(self, stream=None):
-        return tkhp_nblist_atom_stats(self.ctx, stream)
+        return tkhp_nblist_atom_stats(self.ctx, self._s(stream))
 
     def perm_field(self, charge, dipole, quad, out=None, stream=None):
         q, d, th = self._f64(charge), self._f64(dipole), self._f64(quad)
         if out is None:
             out = self.torch.empty((self.n, 3), dtype=self.torch.float64, device=self.device)
-        tkhp_perm_field(self.ctx, q, d, th, out, stream)
+        tkhp_perm_field(self.ctx, q, d, th, out, self._s(stream))
         return out
 
     def tmatvec(self, mu, out=None, stream=None):
         mu = self._f64(mu)
         if out is None:
             out = self.torch.empty((self.n, 3), dtype=self.torch.float64, device=self.device)
-        tkhp_tmatvec(self.ctx, mu, out, stream)
+        tkhp_tmatvec(self.ctx, mu, out, self._s(stream))
         return out
 
     def polar_solve(self, field, tol=1e-6, max_iter=100, guess=None, stream=None,
@@ -340,7 +344,7 @@ class Polarizer:
             mu = self.torch.empty((self.n, 3), dtype=self.torch.float64, device=self.device)
         else:
             mu = self._f64(guess).clone()
-        it, rms, _ = tkhp_polar_solve(self.ctx, field, mu, tol, max_iter, guess is not None, stream,
+        it, rms, _ = tkhp_polar_solve(self.ctx, field, mu, tol, max_iter, guess is not None, self._s(stream),
                                       allow_noconv)
         return mu, it, rms
 

@@ -69,8 +69,7 @@ static size_t carve(Ctx *c, const tkhp_params *p, void *base) {
     const int n_blocks = (int)((n + BLOCK - 1) / BLOCK);
     const size_t n_pad = (size_t)n_blocks * BLOCK;
     const int n_super = (n_blocks + SUPER - 1) / SUPER;
-    int b_alloc = p->box > 0.0 ? grid_bits_for(p->box) : 7;
-    if (p->box <= 0.0 && n < 4096) b_alloc = 5;
+    const int b_alloc = p->box > 0.0 ? grid_bits_for(p->box) : 6;      // open boundary: b <= 6
     size_t n_cells = (size_t)1 << (3 * b_alloc);
     size_t bins = n_cells > n ? n_cells : n;
     const long long cap_tiles = tile_capacity(p, n_blocks);

@@ -198,7 +198,7 @@ __global__ void k_extent(const double *__restrict__ pos, int n, DeviceState *st)
 }
 
 // open boundary only: extent = 1.000001 max_axis(hi-lo) + 1e-9 ; b = smallest 1..b_max with
-// extent / 2^b <= 2.5 ; inv_h = 2^b / extent
+// extent / 2^b <= 2.5, else b_max (= 6 for open boundaries) ; inv_h = 2^b / extent
 __global__ void k_grid_from_extent(DeviceState *st, int b_max) {
     double span = 0.0;
     for (int c = 0; c < 3; ++c) {
@@ -207,8 +207,7 @@ __global__ void k_grid_from_extent(DeviceState *st, int b_max) {
     }
     double extent = __dadd_rn(__dmul_rn(span, 1.000001), 1e-9);
     int b = 1;
-    while (__ddiv_rn(extent, (double)(1 << b)) > 2.5 && b < 8) ++b;
-    if (b > b_max) { b = b_max; st->err_capacity = 1; }
+    while (__ddiv_rn(extent, (double)(1 << b)) > 2.5 && b < b_max) ++b;      // coarser cells beyond b_max: only the sort locality suffers
     st->grid_bits = b;
     st->grid_inv_h = __ddiv_rn((double)(1 << b), extent);
 }

@@ -167,3 +167,50 @@ def test_pair_count_matches_density():
     tot = oracle.count_pairs_rows(s, np.arange(s.n_atoms))
     assert tot == 2 * n_pair
     assert oracle.count_pairs_rows(s, rows) > 0
+
+
+def _brute_force_pairs(pos, box, cutoff):
+    """The definition, written out here in numpy (not through oracle/): unordered pairs i < j with
+    minimum-image R^2 <= r_c^2, and the same count per row."""
+    n = pos.shape[0]
+    d = pos[:, None, :] - pos[None, :, :]
+    if box > 0:
+        d = d - box * np.rint(d / box)
+    r2 = np.einsum("ijk,ijk->ij", d, d)
+    inside = r2 <= cutoff * cutoff
+    np.fill_diagonal(inside, False)
+    return int(np.triu(inside, 1).sum()), inside.sum(axis=1)
+
+
+@pytest.mark.parametrize("periodic", [True, False])
+def test_pair_count_is_exact_against_brute_force(periodic):
+    """SURVEY 8(c) Q7 (R^2 <= r_c^2, inclusive) and Q17 (single minimum image): count_pairs and
+    count_pairs_rows against a numpy brute force, with one pair placed exactly on the cutoff and, in
+    the periodic case, one pair that is only inside r_c through the boundary.  A `<` written for
+    `<=` or a dropped minimum image fails here."""
+    from synth_inputs import tiny_cluster
+    if periodic:
+        s = tiny_cluster(65, 11, box=14.0, spread=14.0, cutoff=5.0, skin=1.0, ewald_beta=0.6)
+    else:
+        s = tiny_cluster(97, 12, box=0.0, spread=12.0, cutoff=5.0, skin=1.0)
+    pos = s.pos.copy()
+    # atoms 0 and 1 exactly r_c apart along x (1.0 and 6.0 are exact in FP64: R^2 == r_c^2 == 25)
+    pos[0] = (1.0, 3.25, 7.5)
+    pos[1] = (6.0, 3.25, 7.5)
+    if periodic:
+        # atoms 2 and 3: 13.0 apart in the box, 1.0 apart through the boundary
+        pos[2] = (0.25, 9.0, 2.0)
+        pos[3] = (13.25, 9.0, 2.0)
+    s = s.with_(pos=pos)
+    n_ref, per_row = _brute_force_pairs(pos, s.box, s.cutoff)
+    d01 = pos[0] - pos[1]
+    assert float(d01 @ d01) == s.cutoff ** 2                   # the edge pair really sits on the edge
+    assert oracle.count_pairs(s) == n_ref
+    rows = np.array([0, 1, 2, 3, 17, 40, s.n_atoms - 1], dtype=np.int64)
+    assert oracle.count_pairs_rows(s, rows) == int(per_row[rows].sum())
+    assert oracle.count_pairs_rows(s, np.arange(s.n_atoms)) == 2 * n_ref == int(per_row.sum())
+    # the edge pair and (periodic) the boundary pair are among the counted ones
+    assert oracle.count_pairs_rows(s, np.array([0])) == int(per_row[0]) >= 1
+    if periodic:
+        no_image = _brute_force_pairs(pos, 0.0, s.cutoff)[0]
+        assert no_image < n_ref                                # the minimum image matters in this system
