@@ -33,11 +33,14 @@ struct SolveArgs {
     ClusterWs ws;
     const float4 *gpos;        // n_pad: own atoms, group frame
     const float4 *stage_pos;   // n_groups * s_cap
-    const float4 *mu0;         // n_pad: the initial guess, packed (k_pcg_init)
+    float4 *mu0;               // n_pad: the initial guess, packed by the owners (sorted order)
     float4 *u32;               // n_pad: u = fp32(alpha r), published by the owners before the barrier that completes r.z
     TmuConsts K;
-    const double *vE;          // 3 n_pad sorted field
-    double *vmu;               // 3 n_pad in: mu0, out: mu
+    const double *field;       // N x 3, caller's order
+    double *mu;                // N x 3, caller's order: in (guess) / out
+    const int32_t *perm;       // n_pad: sorted slot -> caller's atom, -1 = phantom
+    int use_guess;
+    volatile double *result;   // host-mapped: |r|^2, iterations, barrier time-out flag
     const double *alpha_s, *inv_alpha_s;
     double *part_a, *part_b;   // 2 * n_groups each
     DeviceState *st;
@@ -153,17 +156,30 @@ k_pcg_persist(SolveArgs a) {
         s_b[l] = make_float2(0.f, 0.f);
         s_w[l] = p.w;
     }
-    double al = 0.0, ia = 0.0;
+    // the owner's atom in the caller's order; mu0 = alpha E or the caller's guess, published for the
+    // first product (all CTAs gather it after the first grid barrier)
+    double al = 0.0, ia = 0.0, E[3] = {0.0, 0.0, 0.0};
+    const int atom = owner ? a.perm[slot] : -1;
     if (owner) {
         al = a.alpha_s[slot];
         ia = a.inv_alpha_s[slot];
+        double m0[3] = {0.0, 0.0, 0.0};
+        if (atom >= 0) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                E[k] = a.field[3 * (size_t)atom + k];
+                m0[k] = a.use_guess ? a.mu[3 * (size_t)atom + k] : al * E[k];
+            }
+        }
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            s_vec[k * GT + t] = a.vmu[(size_t)k * n_pad + slot];      // mu0
+            s_vec[k * GT + t] = m0[k];
             s_p[k * GT + t] = 0.f;
         }
+        a.mu0[slot] = make_float4((float)m0[0], (float)m0[1], (float)m0[2], 0.f);
     }
     unsigned gen = 0;
+    grid_barrier(st, gen);
     double rz_old = 0.0, rr = 0.0;
     float delta = 0.f;
     int it = 0;                                  // iterations completed
@@ -214,7 +230,7 @@ k_pcg_persist(SolveArgs a) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const double m = s_vec[c * GT + t];
-                    const double r = a.vE[(size_t)c * n_pad + slot] - (m * ia - Tv[c] - a.self * m);
+                    const double r = E[c] - (m * ia - Tv[c] - a.self * m);
                     const double z = al * r;
                     s_vec[(3 + c) * GT + t] = r;
                     uf[c] = (float)z;
@@ -276,15 +292,19 @@ k_pcg_persist(SolveArgs a) {
             for (int c = 0; c < 3; ++c) s_p[c * GT + t] = fmaf(delta, s_p[c * GT + t], uf[c]);
         }
     }
-    // ---- result
-    if (owner) {
+    // ---- result, in the caller's order; the scalars go to host-mapped memory
+    if (owner && atom >= 0) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) a.vmu[(size_t)c * n_pad + slot] = s_vec[c * GT + t];
+        for (int c = 0; c < 3; ++c) a.mu[3 * (size_t)atom + c] = s_vec[c * GT + t];
     }
     if (g == 0 && t == 0) {
         st->rr = rr;
         st->iters = it;
         st->conv_at = converged ? it : 0x7fffffff;
+        a.result[0] = rr;
+        a.result[1] = (double)it;
+        a.result[2] = (double)st->err_barrier;
+        __threadfence_system();
     }
 }
 
@@ -328,8 +348,9 @@ bool atom_solve_eligible(Ctx *c) {
     return (long long)per_sm * c->sm_count >= ws.n_groups && ws.n_groups <= c->part_cap;
 }
 
-// vE, vmu (= mu0) and u32 (= mu0) have been written by k_pcg_init on the same stream.
-int atom_solve_launch(Ctx *c, double tol, int max_iter, cudaStream_t s) {
+// The kernel reads the field (and the guess) and writes mu in the caller's order; |r|^2, the iteration
+// count and the barrier flag arrive in c->h_ring[0..2] (host-mapped) when the stream has drained.
+int atom_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess, double tol, int max_iter, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
     const double b = c->p.ewald_beta;
     SolveArgs a;
@@ -343,8 +364,11 @@ int atom_solve_launch(Ctx *c, double tol, int max_iter, cudaStream_t s) {
     a.K.c1b = (float)(2.0 / SQRT_PI * b);
     a.K.k3 = (float)(4.0 / (3.0 * SQRT_PI) * b * b * b);
     for (int k = 0; k < 6; ++k) a.K.q[k] = c->far_q[k];
-    a.vE = c->vE;
-    a.vmu = c->vmu;
+    a.field = d_field;
+    a.mu = d_mu;
+    a.perm = c->perm;
+    a.use_guess = use_guess;
+    a.result = c->d_ring;
     a.alpha_s = c->alpha_s;
     a.inv_alpha_s = c->inv_alpha_s;
     a.part_a = c->partials;

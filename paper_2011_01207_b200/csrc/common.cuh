@@ -204,7 +204,7 @@ int atom_pairs_configure(Ctx *c);
 int cluster_pairs_configure(Ctx *c);
 int atom_solve_configure(Ctx *c);
 bool atom_solve_eligible(Ctx *c);
-int atom_solve_launch(Ctx *c, double tol, int max_iter, cudaStream_t s);
+int atom_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess, double tol, int max_iter, cudaStream_t s);
 int atom_tmatvec(Ctx *c, cudaStream_t s);
 int atom_field(Ctx *c, cudaStream_t s);
 long long atom_slots(Ctx *c);

@@ -439,31 +439,21 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
             cudaGetLastError();
     }
 
-    // ---- the whole solve as one persistent cooperative kernel (atom_solve.cu) when it can run
+    // ---- the whole solve as one persistent cooperative kernel (atom_solve.cu) when it can run: it
+    // reads the field and the guess and writes mu in the caller's order, the scalars come back
+    // through host-mapped memory
     if (atom_solve_eligible(c)) {
-        k_pcg_init<float4><<<g1, VEC_THREADS, 0, s>>>(d_field, d_mu, use_guess, c->perm, c->alpha_s, n_pad, c->vE, c->vmu, c->mu32, c->st);
-        c->n_launches += 1;
         const bool rec = c->prof && c->prof_n[2] < PROF_MAX;
         if (rec) cudaEventRecord(c->prof_ev[2][2 * c->prof_n[2]], s);
-        rc = atom_solve_launch(c, tol, max_iter, s);
+        rc = atom_solve_launch(c, d_field, d_mu, use_guess, tol, max_iter, s);
         if (rec) { cudaEventRecord(c->prof_ev[2][2 * c->prof_n[2] + 1], s); c->prof_n[2]++; }
-        if (rc) {
-            cudaStreamSynchronize(s);
-            return rc;
-        }
-        k_unsort3<<<g1, VEC_THREADS, 0, s>>>(c->vmu, c->perm, n_pad, d_mu);
-        c->n_launches += 1;
-        TKHP_CUDA(c, cudaGetLastError());
-        TKHP_CUDA(c, cudaMemcpyAsync(c->h_scalars, &c->st->rr, sizeof(double), cudaMemcpyDeviceToHost, s));
-        TKHP_CUDA(c, cudaMemcpyAsync(c->h_scalars + 1, &c->st->iters, sizeof(int), cudaMemcpyDeviceToHost, s));
-        TKHP_CUDA(c, cudaMemcpyAsync(c->h_scalars + 2, &c->st->err_barrier, sizeof(int), cudaMemcpyDeviceToHost, s));
-        TKHP_CUDA(c, cudaStreamSynchronize(s));
-        int it_done, bar_err;
-        memcpy(&it_done, c->h_scalars + 1, sizeof(int));
-        memcpy(&bar_err, c->h_scalars + 2, sizeof(int));
-        if (bar_err) return set_err(c, TKHP_ECUDA, "grid barrier of the persistent PCG kernel timed out%s");
+        const cudaError_t e = cudaStreamSynchronize(s);
+        if (rc) return rc;
+        TKHP_CUDA(c, e);
+        const int it_done = (int)c->h_ring[1];
+        const double rms_done = sqrt(c->h_ring[0] / c->n);
+        if (c->h_ring[2] != 0.0) return set_err(c, TKHP_ECUDA, "grid barrier of the persistent PCG kernel timed out%s");
         if (rec) c->prof_solve_matvecs += it_done + 1;
-        const double rms_done = sqrt(c->h_scalars[0] / c->n);
         if (h_iters) *h_iters = it_done;
         if (h_rms) *h_rms = rms_done;
         if (!(rms_done < tol)) return set_err(c, TKHP_ENOCONV, "PCG did not reach the tolerance within max_iter%s");
