@@ -28,8 +28,8 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
         snprintf(err, n, "cutoff + skin = %g exceeds box/2 = %g (single minimum image)", p->cutoff + p->skin, 0.5 * p->box);
         return TKHP_ECUTOFF;
     }
-    if (p->precision == TKHP_MIXED && p->ewald_beta * p->cutoff > 6.0) {
-        snprintf(err, n, "MIXED precision supports ewald_beta * cutoff <= 6 (erfc fit range)");
+    if (p->ewald_beta * p->cutoff > 6.0) {
+        snprintf(err, n, "ewald_beta * cutoff must be <= 6 (range of the erfc fits)");
         return TKHP_EINVAL;
     }
     if (p->precision == TKHP_MIXED && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }

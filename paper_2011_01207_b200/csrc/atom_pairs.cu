@@ -171,8 +171,9 @@ __device__ __forceinline__ void pair_epilogue(unsigned char *smem_raw, double dx
     }
 }
 
-// resident CTAs per SM the register allocation must allow: FP32 field 2 (112 KB of staging), FP64 1
-template <typename real, int MODE> struct MinCtas { static constexpr int N = sizeof(real) == 8 ? 1 : 2; };
+// resident CTAs per SM the register allocation must allow: FP32 field 2 (112 KB of staging), FP64 T.mu 2
+// (53 KB), FP64 field 1 (106 KB)
+template <typename real, int MODE> struct MinCtas { static constexpr int N = (sizeof(real) == 8 && MODE == MODE_FIELD) ? 1 : 2; };
 
 // ----------------------------------------------------------------------------- generic kernel
 template <typename real, int MODE>

@@ -14,12 +14,14 @@
 //
 // MIXED (float): erfcx by the degree-7 polynomial of erfcx_coeffs.h in u = 1/(1+0.35z)
 // (MUFU.RCP), exponentials by ex2.approx, 1/R by MUFU.RSQ: 4 MUFU + ~45 FMA-pipe ops per pair.
-// FP64 (double): erfc()/exp() of the CUDA math library.
+// FP64 (double): erfcx by a degree-16 polynomial in the same u, exponentials by exp_neg (below);
+// libm only in the FP64 correction pass over the few same-group pairs.
 #pragma once
 
 #include <cuda_runtime.h>
 
 #include "erfcx_coeffs.h"
+#include "erfcx_coeffs64.h"
 
 namespace tkhp {
 
@@ -133,19 +135,47 @@ __device__ __forceinline__ void radial_f32(float r2, float ww, const PairConsts<
 }
 
 // ---- FP64: G_1..G_NK for an unmasked pair --------------------------------------------------
+// libm's erfc() and exp() cost about 250 FP64-pipe instructions per pair; the same scaled form as the
+// FP32 path needs about 90: erfcx(z) by the degree-16 polynomial of erfcx_coeffs64.h in
+// u = 1/(1 + 0.35 z) (5e-15 relative, 0 <= z <= 6) and e^{-y} by exp_neg below (2e-15).
+//
+// e^{y} for y <= 0: y log2(e) = n + f, |f| <= 1/2, 2^f = e^{f ln 2} by its Taylor polynomial of degree
+// 11 (6e-15), scaled by 2^n through the exponent field; 0 below the normal range.
+__device__ __forceinline__ double exp_neg(double y) {
+    constexpr double L2E_HI = 1.4426950408889634, L2E_LO = 2.0355273740931033e-17;
+    const double tq = y * L2E_HI;
+    if (tq < -1020.0) return 0.0;
+    const double n = rint(tq);
+    const double f = fma(y, L2E_HI, -n) + y * L2E_LO;
+    constexpr double c[12] = {1.0, 0.6931471805599453, 0.2402265069591007, 0.05550410866482158,
+                              0.009618129107628477, 0.0013333558146428443, 1.5403530393381608e-4,
+                              1.5252733804059841e-5, 1.3215486790144307e-6, 1.0178086009239699e-7,
+                              7.054911620801123e-9, 4.445538271870811e-10};
+    double p = c[11];
+#pragma unroll
+    for (int k = 10; k >= 0; --k) p = fma(p, f, c[k]);
+    const int hi = __double2hiint(p) + ((int)n << 20);
+    return __hiloint2double(hi, __double2loint(p));
+}
+
 template <int NK>
 __device__ __forceinline__ void radial_f64(double r2, double ww, const PairConsts<double> &k, double *G) {
-    const double r = sqrt(r2);
-    const double rinv = 1.0 / r;
+    constexpr double c[TKHP_ERFCX64_DEG + 1] = TKHP_ERFCX64_COEFFS;
+    const double rinv = rsqrt(r2);
+    const double r = r2 * rinv;
     const double rinv2 = rinv * rinv;
     const double z = k.beta * r;
-    const double ez = exp(-z * z);
-    // R^(2k+1) bn_k by the upward recursion, written in z:  B1 = erfc(z) + c z ez
-    const double cz = k.c1 * z;
     const double z2 = z * z;
-    const double B1 = erfc(z) + cz * ez;
+    const double ez = exp_neg(-z2);
+    // R^(2k+1) bn_k = ez [(2k-1)!! (erfcx(z) + c z) + ...]  (pair_math header)
+    const double u = 1.0 / fma(TKHP_ERFCX64_P, z, 1.0);
+    double p = c[TKHP_ERFCX64_DEG];
+#pragma unroll
+    for (int d = TKHP_ERFCX64_DEG - 1; d >= 0; --d) p = fma(p, u, c[d]);
+    const double cz = k.c1 * z;
+    const double B1 = ez * (p + cz);                       // erfc(z) + c z e^{-z^2}
     const double x = (r2 * r) * ww;
-    const double et = exp(-x);
+    const double et = exp_neg(-x);
     const double rinv3 = rinv2 * rinv;
     G[0] = (B1 - et) * rinv3;
     if (NK >= 2) {

@@ -73,11 +73,14 @@ def test_host_side_parameter_checks(built_lib):
         with pytest.raises(pk.TkhpError) as e:
             pk.tkhp_workspace_bytes(p)
         assert e.value.code == -1, field
-    # MIXED erfc fit range
+    # range of the erfc fits (both precisions): beta * cutoff <= 6
     p = pk.TkhpParams(648, pk.TKHP_MIXED, 0, 0, 40.0, 7.0, 2.0, 1.0, 0.39, 0, 0)
     with pytest.raises(pk.TkhpError):
         pk.tkhp_workspace_bytes(p)
     p.precision = pk.TKHP_FP64
+    with pytest.raises(pk.TkhpError):
+        pk.tkhp_workspace_bytes(p)
+    p.ewald_beta = 0.85
     assert pk.tkhp_workspace_bytes(p) > 0
 
 
