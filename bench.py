@@ -3,6 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
                     [--config 0|1|2|3] [--precision mixed|fp64] [--list-mode auto|tiles|cluster|atom]
+    python bench.py --table [--table-configs 0,1,2,3] [--sweep] [--reps R]
 
 One STEP = one pass of the whole hot path over one synthetic system:
 neighbour-list build -> permanent field -> PCG solve to RMS 1e-6 -> polarization energy
@@ -64,6 +65,12 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--peak-seconds", type=float, default=1.0)
+    ap.add_argument("--table", action="store_true",
+                    help="instead of the JSON line: the markdown result table of BASELINE.md section 3 "
+                         "(every config and precision, errors against the oracle; several minutes)")
+    ap.add_argument("--table-configs", default="0,1,2,3")
+    ap.add_argument("--sweep", action="store_true", help="--table: add config 4 (r_c = 7, 9, 12 A, both precisions)")
+    ap.add_argument("--reps", type=int, default=10)
     return ap.parse_args()
 
 
@@ -172,6 +179,102 @@ def run_reference(args, rank: int, world: int):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- result table
+def _table_rows(s, perm, n_rand, n_blocks, seed=0):
+    rng = np.random.default_rng(seed)
+    rows = set(rng.choice(s.n_atoms, size=min(n_rand, s.n_atoms), replace=False).tolist())
+    nb = perm.size // 32
+    for b in rng.choice(nb, size=min(n_blocks, nb), replace=False):
+        rows.update(int(a) for a in perm[32 * b:32 * b + 32] if a >= 0)
+    rows.update(int(a) for a in perm[-32:] if a >= 0)
+    return np.array(sorted(rows), dtype=np.int64)
+
+
+def _table_one(s, label, precision, reps, full_oracle):
+    """One row of the table: medians of `reps` steps (CUDA events inside the library), the live pair
+    kernel durations, and the errors against the FP64 oracle (the cpu_baseline's oracle, as it stands)."""
+    import torch
+    import oracle
+    import paper_2011_01207_b200 as pk
+    rel = lambda a, b: float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(b))
+    prec = pk.TKHP_FP64 if precision == "fp64" else pk.TKHP_MIXED
+    stream = torch.cuda.Stream()
+    torch.cuda.set_stream(stream)
+    P = pk.Polarizer.for_system(s, precision=prec, list_mode=pk.TKHP_LIST_ATOM)
+    dev = P.device
+    f64 = torch.float64
+    d_pos = torch.as_tensor(s.pos, dtype=f64, device=dev)
+    d_alpha = torch.as_tensor(s.polarizability, dtype=f64, device=dev)
+    d_group = torch.as_tensor(s.group_id, dtype=torch.int32, device=dev)
+    probe = np.random.default_rng(1).standard_normal((s.n_atoms, 3)) * 0.1
+    d_probe = torch.as_tensor(probe, dtype=f64, device=dev)
+    t = dict(build=[], field=[], solve=[], energy=[], tmu=[], fld=[])
+    it = 0
+    for r in range(reps + 2):
+        pk.tkhp_profile_reset(P.ctx, True)
+        pk.tkhp_nblist_build(P.ctx, d_pos, d_alpha, d_group, stream)
+        E = P.perm_field(s.charge, s.dipole, s.quad)
+        mu, it, rms = P.polar_solve(E, tol=1e-6)
+        float(P.polar_energy(mu, E).cpu())
+        P.tmatvec(d_probe)                                  # one stand-alone product: the T.mu pair kernel's time
+        torch.cuda.synchronize()
+        if r < 2:
+            continue
+        ph = P.timings()
+        pr = pk.tkhp_profile_read(P.ctx)
+        for k in ("build", "field", "solve", "energy"):
+            t[k].append(ph[k])
+        t["tmu"].append(pr["tmatvec_ms"] / max(pr["n_tmatvec"], 1))
+        t["fld"].append(pr["field_ms"] / max(pr["n_field"], 1))
+    med = {k: statistics.median(v) for k, v in t.items()}
+    n_pair, n_slots, mode = P.nblist_stats()
+    perm, _ = P.nblist_view()
+    t0 = time.perf_counter()
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    Tg = P.tmatvec(probe).cpu().numpy()
+    gtol = 1e-12 if precision == "fp64" else 1e-8
+    mu_g, _, _ = P.polar_solve(Eg, tol=gtol)
+    e_g = float(P.polar_energy(mu_g, Eg).cpu())
+    if full_oracle:
+        E_ref = oracle.perm_field(s)
+        T_ref = oracle.tmatvec(s, probe)
+        mu_ref, _, _ = oracle.pcg_solve(s, E_ref, tol=1e-10)
+        e_ref = oracle.polar_energy(mu_ref, E_ref)
+        err_txt = "%.1e / %.1e / %.1e, %.1e" % (rel(Tg, T_ref), rel(Eg.cpu().numpy(), E_ref),
+                                                rel(mu_g.cpu().numpy(), mu_ref), abs(e_g - e_ref) / abs(e_ref))
+    else:
+        rows = _table_rows(s, perm, 2048, 8)
+        err_txt = "%.1e / %.1e / -, - (%d sampled rows)" % (rel(Tg[rows], oracle.tmatvec_rows(s, probe, rows)),
+                                                           rel(Eg.cpu().numpy()[rows], oracle.perm_field_rows(s, rows)), rows.size)
+    oracle_s = time.perf_counter() - t0
+    P.close()
+    gp = lambda ms: n_pair / (ms * 1e-3) / 1e9
+    print("| %s | %s | %d | %d | %d | %.3f | %.4f (%.0f) | %.4f (%.0f) | %d | %.3f | %s | %.0f (%d) |" % (
+        label, precision, s.n_atoms, n_pair, n_slots, med["build"], med["fld"], gp(med["fld"]), med["tmu"],
+        gp(med["tmu"]), it, med["solve"], err_txt, oracle_s, oracle.num_threads()), flush=True)
+
+
+def run_table(args):
+    """--table: BASELINE.md section 3's result table (SURVEY 8(d) protocol), markdown rows on stdout."""
+    import oracle
+    from synth_inputs import make_config
+    oracle.build()
+    print("| config | precision | N | N_pair (R <= r_c) | slots evaluated per product | list build ms | field kernel ms "
+          "(G pairs/s) | stand-alone T.mu kernel ms (G pairs/s) | PCG iterations (1e-6) | solve ms | rel-L2 T.mu / E / mu, "
+          "rel E_pol vs oracle | oracle + parity run s (cores) |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for c in [int(x) for x in args.table_configs.split(",") if x != ""]:
+        s = make_config(c)
+        for precision in (("fp64", "mixed") if c < 3 else ("mixed",)):
+            _table_one(s, str(c), precision, args.reps, full_oracle=c < 3)
+    if args.sweep:
+        for rc in (9.0, 12.0):
+            s = make_config(4, cutoff=rc)
+            for precision in ("fp64", "mixed"):
+                _table_one(s, "4, r_c = %g A, beta = %.5f" % (rc, s.ewald_beta), precision, max(3, args.reps // 2),
+                           full_oracle=True)
 
 
 # ----------------------------------------------------------------------------- our arm
@@ -462,7 +565,10 @@ def main():
         from paper_2011_01207_b200 import replicas
         cmd = replicas.torchrun_command(sys.executable, str(Path(__file__).resolve()), args.gpus, sys.argv[1:])
         raise SystemExit(subprocess.call(cmd))
-    if args.impl == "reference":
+    if args.table:
+        if rank == 0:
+            run_table(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, world, local_rank)

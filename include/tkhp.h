@@ -118,8 +118,17 @@ const char *tkhp_last_error(const tkhp_ctx *ctx);
  * Steps: wrap, Hilbert cell key on a 2^b grid, stable sort by (key, index), gather to
  * block-local structure-of-arrays, per-block bounding boxes, block pairs (I <= J) with
  * box gap^2 <= (cutoff+skin)^2 (FP64, no FMA contraction: DESIGN.md section 3), and, in
- * CLUSTER mode, the filtered cluster->atom lists at r_c.  The positions passed here are
- * the positions every later call on this context uses.
+ * CLUSTER and ATOM mode, the filtered cluster->atom lists and the exact per-atom lists
+ * at r_c.  The positions passed here are the positions every later call on this context
+ * uses.
+ * Coincident atoms: the finer lists identify an atom with itself by R^2 <= 1e-10 A^2, so
+ * two DISTINCT atoms closer than 1e-5 A do not interact in CLUSTER/ATOM mode (they would
+ * give 1/0 in the pair formulas; the TILES kernels and the oracle skip only i == j).
+ * Polarization groups are expected to be small (molecules): the mask-correction pass
+ * walks all mates of an atom's group on one thread.
+ * On a stream of the caller's (not the legacy default stream 0) the whole build is
+ * captured once into a CUDA graph, keyed by the three input pointers, and replayed by
+ * later calls with the same pointers; contents may change freely between calls.
  */
 int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polarizability,
                       const int32_t *d_group_id, void *stream);

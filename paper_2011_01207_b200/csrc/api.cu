@@ -158,6 +158,17 @@ static void toc(Ctx *c, int phase, cudaStream_t s) { cudaEventRecord(c->ev[2 * p
 
 using namespace tkhp;
 
+// Every entry point runs with the context's device current and leaves the caller's current device
+// as it found it (a process may hold contexts on several GPUs).
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) cudaSetDevice(dev); else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 extern "C" {
 
 int tkhp_workspace_bytes(const tkhp_params *params, size_t *bytes) {
@@ -182,6 +193,8 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
         cudaGetLastError();
         return TKHP_ECUDA;
     }
+    int prev_device = -1;
+    cudaGetDevice(&prev_device);
     if (cudaSetDevice(params->device) != cudaSuccess) { snprintf(g_create_err, sizeof(g_create_err), "cudaSetDevice failed"); return TKHP_ECUDA; }
     Ctx *c = new (std::nothrow) Ctx();
     if (!c) return TKHP_EINVAL;
@@ -225,7 +238,9 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     c->built = false;
     c->header_valid = false;
     c->list_mode_in_use = TKHP_LIST_TILES;
-    if (cudaDeviceSynchronize() != cudaSuccess) { delete c; return TKHP_ECUDA; }
+    // the device-resident scalars start from zero (tickets, barrier words: tkhp_polar_energy may be the first call)
+    if (cudaMemset(c->st, 0, sizeof(DeviceState)) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) { delete c; return TKHP_ECUDA; }
+    if (prev_device >= 0 && prev_device != params->device) cudaSetDevice(prev_device);      // leave the caller's current device as it was
     *out = reinterpret_cast<tkhp_ctx *>(c);
     return TKHP_OK;
 }
@@ -233,7 +248,7 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
 int tkhp_destroy(tkhp_ctx *ctx) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
-    cudaSetDevice(c->p.device);
+    DeviceGuard guard(c->p.device);
     cudaDeviceSynchronize();
     for (int i = 0; i < 10; ++i) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 2; ++i) cudaEventDestroy(c->copy_ev[i]);
@@ -273,6 +288,7 @@ int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polari
                       const int32_t *d_group_id, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     if (!d_pos || !d_polarizability || !d_group_id) return set_err(c, TKHP_EINVAL, "NULL input%s");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     tic(c, 0, s);
@@ -321,6 +337,7 @@ int tkhp_nblist_view(tkhp_ctx *ctx, int32_t *n_blocks, int64_t *n_pairs, const i
                      const int32_t **d_pairs, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     int rc = ensure_header(c, static_cast<cudaStream_t>(stream));
     if (rc) return rc;
     if (n_blocks) *n_blocks = c->n_blocks;
@@ -334,6 +351,7 @@ int tkhp_nblist_stats(tkhp_ctx *ctx, int64_t *n_pairs_within_cutoff, int64_t *n_
                       int32_t *list_mode_in_use, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = ensure_header(c, s);
     if (rc) return rc;
@@ -363,6 +381,7 @@ int tkhp_nblist_stats(tkhp_ctx *ctx, int64_t *n_pairs_within_cutoff, int64_t *n_
 int tkhp_nblist_atom_stats(tkhp_ctx *ctx, int64_t out[4], void *stream) {
     if (!ctx || !out) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     int rc = ensure_header(c, static_cast<cudaStream_t>(stream));
     if (rc) return rc;
     out[0] = out[1] = out[2] = out[3] = 0;
@@ -379,6 +398,7 @@ int tkhp_perm_field(tkhp_ctx *ctx, const double *d_charge, const double *d_dipol
                     double *d_field, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     if (!d_charge || !d_dipole || !d_quad || !d_field) return set_err(c, TKHP_EINVAL, "NULL argument%s");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = ensure_header(c, s);
@@ -392,6 +412,7 @@ int tkhp_perm_field(tkhp_ctx *ctx, const double *d_charge, const double *d_dipol
 int tkhp_tmatvec(tkhp_ctx *ctx, const double *d_mu, double *d_out, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     if (!d_mu || !d_out || d_mu == d_out) return set_err(c, TKHP_EINVAL, "NULL or aliased argument%s");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = ensure_header(c, s);
@@ -406,6 +427,7 @@ int tkhp_polar_solve(tkhp_ctx *ctx, const double *d_field, double *d_mu, double 
                      int32_t use_guess, int32_t *h_iters, double *h_rms, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     if (!d_field || !d_mu || !(tol > 0.0) || max_iter < 0) return set_err(c, TKHP_EINVAL, "bad argument%s");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     int rc = ensure_header(c, s);
@@ -419,6 +441,7 @@ int tkhp_polar_solve(tkhp_ctx *ctx, const double *d_field, double *d_mu, double 
 int tkhp_polar_energy(tkhp_ctx *ctx, const double *d_mu, const double *d_field, double *d_energy, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     if (!d_mu || !d_field || !d_energy) return set_err(c, TKHP_EINVAL, "NULL argument%s");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     tic(c, 4, s);
@@ -433,6 +456,7 @@ int tkhp_polarize_host(tkhp_ctx *ctx, const double *h_pos, const double *h_polar
                        double *h_energy, int32_t *h_iters, double *h_rms, void *stream) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     if (!h_pos || !h_polarizability || !h_group_id || !h_charge || !h_dipole || !h_quad || !h_energy)
         return set_err(c, TKHP_EINVAL, "NULL argument%s");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -467,6 +491,7 @@ int tkhp_polarize_host(tkhp_ctx *ctx, const double *h_pos, const double *h_polar
 int tkhp_profile_reset(tkhp_ctx *ctx, int32_t enable_kernel_events) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     c->n_launches = 0;
     c->n_noop_launches = 0;
     c->prof = enable_kernel_events != 0;
@@ -479,6 +504,7 @@ int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmat
                       double *tmatvec_kernel_ms, int32_t *n_field_kernels, double *field_kernel_ms) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     if (n_kernel_launches) *n_kernel_launches = c->n_launches - c->n_noop_launches;
     double tot[2] = {0.0, 0.0};
     int cnt[2] = {0, 0};
@@ -505,6 +531,7 @@ int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmat
 int tkhp_profile_read_solve(tkhp_ctx *ctx, int32_t *n_solve_kernels, double *solve_kernel_ms, int64_t *n_matvecs) {
     if (!ctx) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     double tot = 0.0;
     for (int i = 0; i < c->prof_n[2]; ++i) {
         float t = 0.f;
@@ -524,6 +551,7 @@ int tkhp_profile_read_solve(tkhp_ctx *ctx, int32_t *n_solve_kernels, double *sol
 int tkhp_last_timings(tkhp_ctx *ctx, double ms[5]) {
     if (!ctx || !ms) return TKHP_EINVAL;
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
+    DeviceGuard guard(c->p.device);
     for (int ph = 0; ph < 5; ++ph) {
         if (c->last_ms[ph] < 0.0) { ms[ph] = -1.0; continue; }
         float t = 0.f;

@@ -383,7 +383,8 @@ int atom_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess
     a.rot_div = c->sm_count;
     TKHP_CUDA(c, cudaMemsetAsync(&c->st->bar_count, 0, 2 * sizeof(unsigned), s));
     void *args[] = {&a};
-    TKHP_CUDA(c, cudaLaunchCooperativeKernel(pick(c, ws), dim3(ws.n_groups), dim3(GT), args, solve_smem(a.s_chunk, c->n_blocks / ws.n_groups < 5), s));
+    if (cudaLaunchCooperativeKernel(pick(c, ws), dim3(ws.n_groups), dim3(GT), args, solve_smem(a.s_chunk, c->n_blocks / ws.n_groups < 5), s) != cudaSuccess)
+        return set_err(c, TKHP_ECUDA, "cooperative launch of the persistent PCG kernel was refused%s");
     c->n_launches += 1;
     return TKHP_OK;
 }

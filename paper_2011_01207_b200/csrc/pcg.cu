@@ -91,7 +91,7 @@ __global__ void k_field_finish(const double *__restrict__ acc, const int32_t *__
             Rx -= box * rint(Rx / box); Ry -= box * rint(Ry / box); Rz -= box * rint(Rz / box);
         }
         const double r2 = Rx * Rx + Ry * Ry + Rz * Rz;
-        if (r2 > rc2) continue;
+        if (r2 > rc2 || r2 <= 1e-20) continue;              // (coincident group mates: no 1/0)
         double G[3];
         radial_masked_f64(r2, beta, G);
         const double *d = dip + 3 * (size_t)b;
@@ -448,6 +448,13 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
         rc = atom_solve_launch(c, d_field, d_mu, use_guess, tol, max_iter, s);
         if (rec) { cudaEventRecord(c->prof_ev[2][2 * c->prof_n[2] + 1], s); c->prof_n[2]++; }
         const cudaError_t e = cudaStreamSynchronize(s);
+        if (rc == TKHP_ECUDA && e == cudaSuccess) {
+            // the cooperative launch itself was refused: launch-per-matvec path, now and later
+            cudaGetLastError();
+            c->no_persist = true;
+            if (rec) c->prof_n[2]--;
+            return do_polar_solve(c, d_field, d_mu, tol, max_iter, use_guess, h_iters, h_rms, s);
+        }
         if (rc) return rc;
         TKHP_CUDA(c, e);
         const int it_done = (int)c->h_ring[1];
@@ -486,7 +493,7 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
             rc = run_tmatvec(c, s);
             c->spec_iter = -1;
             c->fuse_q = false;
-            if (rc) return rc;
+            if (rc) { cudaStreamSynchronize(s); return rc; }
             if (!fused_q) {
                 k_pcg_q<<<gv, VEC_THREADS, 0, s>>>(c->acc, c->vp, c->inv_alpha_s, self, n_pad, c->vq, part_pq, c->st, enq);
                 c->n_launches += 1;
@@ -499,9 +506,17 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
                 volatile double *a_ring = c->d_ring + slot;
                 void *args[] = {&a_vp, &a_vq, &a_al, &a_n, &a_mu, &a_r, &a_pk, &a_part, &a_st, &a_it, &a_tol, &a_na, &a_ring};
                 const void *fn = mixed ? (const void *)k_pcg_step<float4> : (const void *)k_pcg_step<double4>;
-                TKHP_CUDA(c, cudaLaunchCooperativeKernel(fn, dim3(g1), dim3(VEC_THREADS), args, 0, s));
-                c->n_launches += 1;
-            } else {
+                if (cudaLaunchCooperativeKernel(fn, dim3(g1), dim3(VEC_THREADS), args, 0, s) == cudaSuccess) {
+                    c->n_launches += 1;
+                } else {
+                    // e.g. cudaErrorCooperativeLaunchTooLarge under MPS / SM partitioning: the two-kernel
+                    // form from this iteration on (nothing of this iteration has been enqueued yet)
+                    cudaGetLastError();
+                    fused_step = false;
+                    c->no_fused_step = true;
+                }
+            }
+            if (!fused_step) {
                 k_pcg_update<<<gv, VEC_THREADS, 0, s>>>(c->vp, c->vq, c->alpha_s, n_pad, c->vmu, c->vr, part_rz, c->st, enq, tol, c->n, c->d_ring + slot);
                 if (mixed)
                     k_pcg_direction<float4><<<gv, VEC_THREADS, 0, s>>>(c->vr, c->alpha_s, n_pad, c->vp, c->mu32, c->st, enq);
@@ -511,7 +526,7 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
             }
             ++enq;
         }
-        if ((rc = wait_slot(c, s, seen % RING, &rr))) return rc;
+        if ((rc = wait_slot(c, s, seen % RING, &rr))) { cudaStreamSynchronize(s); return rc; }
         it = seen++;                                // iterations completed when this residual was formed
         rms = sqrt(rr / c->n);
         if (rms < tol || !(rms == rms) || it >= max_iter) break;
