@@ -57,8 +57,26 @@ __device__ __forceinline__ void deal(Deal &d, uint16_t *img, int colcap, unsigne
 // rows of column j that lie inside a list of `len` entries
 __device__ __forceinline__ unsigned col_cap(unsigned j, unsigned len) { return j < len ? (len - j + 15u) >> 4 : 0u; }
 
-// entries of over-full columns -> holes of under-full ones (per lane, no cross-lane traffic)
+// Entries of over-full columns -> holes of under-full ones (per lane, no cross-lane traffic).  First
+// into the PARTNER column (j + 8) mod 16: its steps want the same index class mod 8, so the quarter
+// warp's LDS.128 stays conflict-free and only the half warp's LDS.64 takes a second wavefront; what
+// is left goes into any hole (those steps may conflict with one other lane).
 __device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16, unsigned len) {
+    // pass 1: partner columns
+    for (unsigned b = 0; b < 16; ++b) {
+        const unsigned j = (b - l16) & 15u, pb = (b + 8u) & 15u, pj = (pb - l16) & 15u;
+        unsigned cb = d.cnt[b * 32], cp = d.cnt[pb * 32];
+        const unsigned capb = col_cap(j, len), capp = col_cap(pj, len);
+        while (cb > capb && cp < capp) {
+            --cb;
+            img[(pj + 16u * cp) * 32] = img[(j + 16u * cb) * 32];
+            img[(j + 16u * cb) * 32] = 0xffffu;
+            ++cp;
+        }
+        d.cnt[b * 32] = (uint8_t)cb;
+        d.cnt[pb * 32] = (uint8_t)cp;
+    }
+    // pass 2: whatever is still over the edge, into the holes in column order
     unsigned hb = 0, hr = d.cnt[0];
     for (unsigned b = 0; b < 16; ++b) {
         const unsigned j = (b - l16) & 15u;
@@ -226,7 +244,7 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
 constexpr int DEAL_WARPS = 4;
 
 __global__ void __launch_bounds__(DEAL_WARPS * 32)
-k_atom_deal(ClusterWs ws, int n_blocks) {
+k_atom_deal(ClusterWs ws, int n_blocks, int rec_bytes) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int blk = blockIdx.x * DEAL_WARPS + w;
@@ -239,7 +257,9 @@ k_atom_deal(ClusterWs ws, int n_blocks) {
     const unsigned l16 = (unsigned)lane & 15u;
     uint4 *__restrict__ rows = reinterpret_cast<uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
     const int2 *__restrict__ seg = ws.aseg + (size_t)blk * NSEG_MAX;
-    const unsigned dummy = (unsigned)seg[NSEG_MAX - 1].y;
+    const unsigned dummy = (unsigned)seg[NSEG_MAX - 1].y;            // byte offset of the first dummy record
+    const bool multi = rec_bytes == 16;                              // 16-byte records: one dummy per index class (N_DUMMY)
+    const unsigned n_loc = dummy / (unsigned)rec_bytes;
     for (int r = 0; r < img_rows; ++r) img[r * 32] = 0xffffu;
     D.clear();
 
@@ -262,7 +282,7 @@ k_atom_deal(ClusterWs ws, int n_blocks) {
                                        e.z & 0xffffu, e.z >> 16, e.w & 0xffffu, e.w >> 16};
 #pragma unroll
                 for (int h = 0; h < 8; ++h)
-                    if (v[h] != dummy) deal(D, img, colcap, l16, v[h], (v[h] >> 4) & 15u);
+                    if (v[h] < dummy) deal(D, img, colcap, l16, v[h], (v[h] >> 4) & 15u);      // (the scan pads with the first dummy)
             }
             level(D, img, l16, (unsigned)len);
             for (int q = 0; q < nrow; ++q) {
@@ -271,7 +291,9 @@ k_atom_deal(ClusterWs ws, int n_blocks) {
                 for (int h = 0; h < 8; ++h) {
                     const int e = 8 * q + h;
                     const unsigned x = img[e * 32];
-                    v[h] = (e >= len || x == 0xffffu) ? dummy : x;
+                    // padding: the dummy record of the index class this lane wants at this step
+                    const unsigned pad = multi ? dummy + (((unsigned)(e + lane) - n_loc) & 15u) * 16u : dummy;
+                    v[h] = (e >= len || x == 0xffffu) ? pad : x;
                     img[e * 32] = 0xffffu;
                 }
                 p[(size_t)q * 32] = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
@@ -303,7 +325,7 @@ int atom_build(Ctx *c, cudaStream_t s) {
     else
         k_atom_scan<float><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos32, ws.stage_pos32, (float)rc2, (float)x2,
                                                           (float)r2_far, s_chunk, c->st);
-    k_atom_deal<<<div_up(c->n_blocks, DEAL_WARPS), DEAL_WARPS * 32, deal_smem(ws), s>>>(ws, c->n_blocks);
+    k_atom_deal<<<div_up(c->n_blocks, DEAL_WARPS), DEAL_WARPS * 32, deal_smem(ws), s>>>(ws, c->n_blocks, f64 ? 32 : 16);
     c->n_launches += 2;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;

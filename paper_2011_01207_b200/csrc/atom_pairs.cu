@@ -188,9 +188,9 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
     constexpr int SU = sizeof(real) == 8 ? 4 : 8;   // staged records in flight per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk + 1]; the dummy follows the group's largest chunk
-    vec4 *s_pay = s_pos + (s_chunk + 1);                       // NPAY arrays of [s_chunk + 1]
-    const int pstride = s_chunk + 1;
+    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk + N_DUMMY]; the dummies follow the group's largest chunk
+    vec4 *s_pay = s_pos + (s_chunk + N_DUMMY);                 // NPAY arrays of [s_chunk + N_DUMMY]
+    const int pstride = s_chunk + N_DUMMY;
     const int pay_stride = pstride * (int)sizeof(vec4);
 
     const int g = blockIdx.x, t = threadIdx.x, lane = t & 31, w = t >> 5;
@@ -214,11 +214,11 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     Partial<real> A;
     int since_flush = 0;
 
-    if (t == 0) {                              // permanent dummy record: far away, zero payload
+    if (t < N_DUMMY) {                         // permanent dummy records: far away, zero payload
         vec4 far, zero;
         far.x = far.y = far.z = (real)(-2.0f * PHANTOM_FAR); far.w = 0;
         zero.x = zero.y = zero.z = zero.w = 0;
-        const int dmy = atom_dummy_index(count, n_chunks);
+        const int dmy = atom_dummy_index(count, n_chunks) + t;
         s_pos[dmy] = far;
         for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + dmy] = zero;
     }
@@ -304,7 +304,7 @@ k_atom_tmu32(ClusterWs ws, const float4 *__restrict__ gpos, const float4 *__rest
     if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     constexpr int SU = 4;                              // staged records in flight per thread
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int pstride = s_chunk + 1;                   // the dummy record follows the group's largest chunk
+    const int pstride = s_chunk + N_DUMMY;             // the dummy records follow the group's largest chunk
     float4 *s_a = reinterpret_cast<float4 *>(smem_raw);
     float2 *s_b = reinterpret_cast<float2 *>(smem_raw + (size_t)16 * pstride);
     float *s_w = reinterpret_cast<float *>(smem_raw + (size_t)24 * pstride);
@@ -335,9 +335,9 @@ k_atom_tmu32(ClusterWs ws, const float4 *__restrict__ gpos, const float4 *__rest
     double dx = 0.0, dy = 0.0, dz = 0.0;
     PartialTmu A;
 
-    if (t == 0) {                              // permanent dummy record: far away, zero payload
+    if (t < N_DUMMY) {                         // permanent dummy records: far away, zero payload
         const float far = -2.0f * PHANTOM_FAR;
-        const int dmy = atom_dummy_index(count, n_chunks);
+        const int dmy = atom_dummy_index(count, n_chunks) + t;
         s_a[dmy] = make_float4(far, far, far, 0.f);
         s_b[dmy] = make_float2(0.f, 0.f);
         s_w[dmy] = 0.f;
@@ -434,7 +434,7 @@ static int launch_atom_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     constexpr int NPAY = MODE == MODE_TMU ? 1 : 3;
     constexpr int which = sizeof(real) == 8;
     const int s_chunk = atom_chunk_capacity(which, ws.chunk_cap);
-    const size_t smem = sizeof(vec4) * (size_t)(1 + NPAY) * (size_t)(s_chunk + 1);
+    const size_t smem = sizeof(vec4) * (size_t)(1 + NPAY) * (size_t)(s_chunk + N_DUMMY);
     PairConsts<real> k;
     k.beta = (real)c->p.ewald_beta;
     k.c1 = (real)(2.0 / SQRT_PI);
@@ -488,7 +488,7 @@ static int launch_tmu32(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
 // dynamic shared memory opt-in of every ATOM-mode pair kernel, once per context (the attribute is
 // per device; tkhp_create calls this with the context's device current)
 int atom_pairs_configure(Ctx *c) {
-    const int big = 2 * ATOM_SMEM + 4096;
+    const int big = 2 * ATOM_SMEM + 8192;
     TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_pairs<float, MODE_FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_pairs<double, MODE_TMU>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));
     TKHP_CUDA(c, cudaFuncSetAttribute(k_atom_pairs<double, MODE_FIELD>, cudaFuncAttributeMaxDynamicSharedMemorySize, big));

@@ -53,21 +53,18 @@ __device__ __forceinline__ unsigned ld_acquire(const unsigned *p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-__device__ __forceinline__ void st_release(unsigned *p, unsigned v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-// All threads of all CTAs.  `gen` counts the barriers this CTA has passed.
+// All threads of all CTAs.  `gen` counts the barriers this CTA has passed.  One atomic per CTA on a
+// counter that only grows during a solve; everybody spins on the counter itself (one L2 round trip
+// less on the critical path than a separate release word written by the last arriver).
 __device__ __forceinline__ void grid_barrier(DeviceState *st, unsigned &gen) {
     __syncthreads();
     ++gen;
     if (threadIdx.x == 0) {
         __threadfence();
-        const unsigned arrived = atomicAdd(&st->bar_count, 1u) + 1u;
-        if (arrived == gen * gridDim.x) st_release(&st->bar_release, gen);
-        else {
+        const unsigned target = gen * gridDim.x;
+        if (atomicAdd(&st->bar_count, 1u) + 1u != target) {
             // bounded spin (a few seconds): a CTA that never arrives must not hang the device
-            for (unsigned n = 0; ld_acquire(&st->bar_release) < gen; ++n)
+            for (unsigned n = 0; ld_acquire(&st->bar_count) < target; ++n)
                 if (n > (1u << 22)) { st->err_barrier = 1; break; }
         }
         __threadfence();
@@ -90,7 +87,7 @@ __device__ __forceinline__ void grid_totals(const double *part, double &a, doubl
 }
 
 __host__ __device__ inline size_t solve_smem(int s_chunk, bool split) {
-    size_t b = ((size_t)TMU_REC * (s_chunk + 1) + 15) & ~(size_t)15;   // A, B, W
+    size_t b = ((size_t)TMU_REC * (s_chunk + N_DUMMY) + 15) & ~(size_t)15;   // A, B, W
     b += (size_t)4 * s_chunk;                                         // staging indices
     b = (b + 15) & ~(size_t)15;
     if (split) b += (size_t)GB * 96 * sizeof(double);                 // parts of a shared block
@@ -103,7 +100,7 @@ template <bool FAR, bool SPLIT>
 __global__ void __launch_bounds__(GT, 3)
 k_pcg_persist(SolveArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int s_chunk = a.s_chunk, pstride = s_chunk + 1;
+    const int s_chunk = a.s_chunk, pstride = s_chunk + N_DUMMY;
     float4 *s_a = reinterpret_cast<float4 *>(smem_raw);
     float2 *s_b = reinterpret_cast<float2 *>(smem_raw + (size_t)16 * pstride);
     float *s_w = reinterpret_cast<float *>(smem_raw + (size_t)24 * pstride);
@@ -143,11 +140,11 @@ k_pcg_persist(SolveArgs a) {
         L.wl = pi.w * 1.4426950408889634f;
     }
     // ---- once per solve: positions, Thole factors, staging indices; the operand slots start at 0
-    if (t == 0) {
+    if (t < N_DUMMY) {
         const float far = -2.0f * PHANTOM_FAR;
-        s_a[count] = make_float4(far, far, far, 0.f);      // the dummy record follows the (only) chunk
-        s_b[count] = make_float2(0.f, 0.f);
-        s_w[count] = 0.f;
+        s_a[count + t] = make_float4(far, far, far, 0.f);      // the dummy records follow the (only) chunk
+        s_b[count + t] = make_float2(0.f, 0.f);
+        s_w[count + t] = 0.f;
     }
     for (int l = t; l < count; l += GT) {
         const float4 p = a.stage_pos[gbase + l];

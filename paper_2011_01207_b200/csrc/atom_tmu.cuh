@@ -133,7 +133,7 @@ __device__ __forceinline__ void tmu_near2(const TmuSmem &S, unsigned off0, unsig
 
 constexpr int TMU_REC = 28;          // staged bytes per record: A 16 + B 8 + W 4
 
-__host__ __device__ inline size_t tmu32_smem(int s_chunk) { return ((size_t)TMU_REC * (s_chunk + 1) + 15) & ~(size_t)15; }
+__host__ __device__ inline size_t tmu32_smem(int s_chunk) { return ((size_t)TMU_REC * (s_chunk + N_DUMMY) + 15) & ~(size_t)15; }
 
 // One row (8 entries per lane) of FAR or NEAR pairs; n < 4: the last row of a class.
 template <bool FARF>

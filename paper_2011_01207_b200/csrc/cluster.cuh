@@ -53,7 +53,11 @@ __host__ __device__ inline int atom_chunk_capacity(bool f64, int user_cap) {
 __host__ __device__ inline int atom_chunks_of(int count, int s_chunk) {
     return count < 1 ? 1 : (count + s_chunk - 1) / s_chunk;
 }
-// local index of the dummy record of a group: one past its largest chunk (<= s_chunk)
+// Padding entries point at DUMMY records (far away, zero payload) that follow the group's largest
+// chunk: N_DUMMY of them, one per index class mod 16, so that a padding entry can be given the class
+// its lane wants at that step (atom_lists.cu: no bank conflict with the lanes that read real records).
+constexpr int N_DUMMY = 16;
+// local index of the first dummy record of a group: one past its largest chunk (<= s_chunk)
 __host__ __device__ inline int atom_dummy_index(int count, int n_chunks) {
     return count < 1 ? 0 : (count + n_chunks - 1) / n_chunks;
 }
