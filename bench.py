@@ -59,7 +59,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3])
-    ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64"])
+    ap.add_argument("--precision", default="mixed", choices=["mixed", "fp64", "fixed"])
     ap.add_argument("--list-mode", default="auto", choices=["auto", "tiles", "cluster", "atom"])
     ap.add_argument("--tol", type=float, default=1e-6)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -301,7 +301,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 
     sys_ = make_config(args.config)
     n = sys_.n_atoms
-    precision = pk.TKHP_MIXED if args.precision == "mixed" else pk.TKHP_FP64
+    precision = {"mixed": pk.TKHP_MIXED, "fp64": pk.TKHP_FP64, "fixed": pk.TKHP_FIXED}[args.precision]
     want_mode = {"auto": pk.TKHP_LIST_ATOM, "atom": pk.TKHP_LIST_ATOM, "cluster": pk.TKHP_LIST_CLUSTER,
                  "tiles": pk.TKHP_LIST_TILES}[args.list_mode]
     mode_name = {pk.TKHP_LIST_TILES: "tiles", pk.TKHP_LIST_CLUSTER: "cluster", pk.TKHP_LIST_ATOM: "atom"}
@@ -409,7 +409,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             sm_ghz = clocks["sm_max_mhz"] / 1e3
     lanes_per_s = sm_count * FP32_LANES_PER_SM * sm_ghz * 1e9
     peak32 = 2 * lanes_per_s / 1e12
-    peak = peak32 if args.precision == "mixed" else peak32 / 2
+    peak = peak32 / 2 if args.precision == "fp64" else peak32
     fld_ms = prof_tot["field_ms"] / max(prof_tot["n_field"], 1)
     persistent = prof_tot["n_solve"] > 0
     if persistent:
@@ -448,7 +448,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "call_ms": phase_stats["tmatvec"],
         },
     }
-    if mode_in_use == pk.TKHP_LIST_ATOM and args.precision == "mixed":
+    if mode_in_use == pk.TKHP_LIST_ATOM and args.precision != "fp64":
         far, near, segs, far_on = P.nblist_atom_stats()
         if not far_on:
             near, far = far + near, 0
@@ -536,7 +536,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32 pair math, f64 accumulation" if args.precision == "mixed" else "f64",
+        "dtype": {"mixed": "f32 pair math, f64 accumulation", "fp64": "f64",
+                  "fixed": "f32 pair math, int64 fixed-point accumulation"}[args.precision],
         "data": "synthetic",
         "config": {"workload": WORKLOADS[args.config], "n_atoms": n, "box": sys_.box,
                    "cutoff": sys_.cutoff, "skin": sys_.skin, "ewald_beta": sys_.ewald_beta,

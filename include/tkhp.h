@@ -54,7 +54,11 @@ enum {
 /* precision of the pair arithmetic (DP and MP modes) */
 enum {
     TKHP_FP64 = 0,  /* every operation in FP64 */
-    TKHP_MIXED = 1  /* FP32 pair math, FP64 accumulation of fields and of all dot products */
+    TKHP_MIXED = 1, /* FP32 pair math, FP64 accumulation of fields and of all dot products */
+    TKHP_FIXED = 2  /* the paper's FP mode (eqs 2-3): FP32 pair math as in MIXED, the
+                       64-bit containers of the pair kernels are INTEGERS, a = int(round(x 2^fB)) with
+                       fB = 34 fractional bits for the field and T.mu accumulators and 30 for the
+                       energy (round = to nearest); PCG dot products stay FP64 tree reductions */
 };
 
 /* which pair-list the compute kernels walk (both are built from the same 32-atom blocks) */

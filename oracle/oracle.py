@@ -35,7 +35,8 @@ __all__ = [
     "count_pairs", "count_pairs_rows", "pcg_solve", "dense_solve",
     "polar_energy", "COULOMB", "wrap", "grid_bits", "cell_coords",
     "hilbert_key", "sort_keys", "check_perm", "block_boxes", "block_pairs",
-    "atom_pairs_covered", "num_threads",
+    "atom_pairs_covered", "num_threads", "to_fixed", "from_fixed", "FIX_VEC_BITS", "FIX_ENERGY_BITS",
+    "OPEN_MAX_BITS",
 ]
 
 _HERE = Path(__file__).resolve().parent
@@ -263,6 +264,21 @@ def dense_solve(sys_, E) -> np.ndarray:
 def polar_energy(mu, E) -> float:
     """(U) E_pol = -1/2 f sum_i mu_i . E_i, f = 332.063713 kcal A / (mol e^2)."""
     return float(-0.5 * COULOMB * np.sum(_f64(mu) * _f64(E)))
+
+
+# ------------------------------------------------------------------ fixed point (paper eqs 2-3)
+FIX_VEC_BITS = 34       # P:L287 "a 34 fractional bits has been selected for forces accumulation"
+FIX_ENERGY_BITS = 30    # P:L287 "For the energy, we only allocated 30 fractional bits"
+
+
+def to_fixed(x, frac_bits: int) -> np.ndarray:
+    """Paper eq. (2): a = int(round(x * 2^fB)); round = to the nearest integer (ties to even)."""
+    return np.rint(np.asarray(x, dtype=np.float64) * float(1 << frac_bits)).astype(np.int64)
+
+
+def from_fixed(a, frac_bits: int) -> np.ndarray:
+    """Paper eq. (3): x = real(a) / 2^fB."""
+    return np.asarray(a, dtype=np.int64).astype(np.float64) / float(1 << frac_bits)
 
 
 # ------------------------------------------------------------------ N

@@ -9,7 +9,7 @@ from pathlib import Path
 TKHP_OK = 0
 TKHP_EINVAL, TKHP_ECUDA, TKHP_ECUTOFF, TKHP_ENOLIST = -1, -2, -3, -4
 TKHP_ENOCONV, TKHP_ECAPACITY, TKHP_ENONFINITE = -5, -6, -7
-TKHP_FP64, TKHP_MIXED = 0, 1
+TKHP_FP64, TKHP_MIXED, TKHP_FIXED = 0, 1, 2
 TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM = 0, 1, 2
 TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP = 1, 2
 

@@ -18,7 +18,7 @@ static int grid_bits_for(double extent) {
 static int check_params(const tkhp_params *p, char *err, size_t n) {
     if (!p) { snprintf(err, n, "params is NULL"); return TKHP_EINVAL; }
     if (p->n_atoms < 1) { snprintf(err, n, "n_atoms must be >= 1"); return TKHP_EINVAL; }
-    if (p->precision != TKHP_FP64 && p->precision != TKHP_MIXED) { snprintf(err, n, "bad precision"); return TKHP_EINVAL; }
+    if (p->precision != TKHP_FP64 && p->precision != TKHP_MIXED && p->precision != TKHP_FIXED) { snprintf(err, n, "bad precision"); return TKHP_EINVAL; }
     if (p->list_mode != TKHP_LIST_TILES && p->list_mode != TKHP_LIST_CLUSTER && p->list_mode != TKHP_LIST_ATOM) { snprintf(err, n, "bad list_mode"); return TKHP_EINVAL; }
     if (!(p->cutoff > 0.0) || !(p->skin >= 0.0) || !isfinite(p->cutoff) || !isfinite(p->skin)) { snprintf(err, n, "cutoff must be > 0 and skin >= 0"); return TKHP_EINVAL; }
     if (!(p->ewald_beta >= 0.0) || !isfinite(p->ewald_beta)) { snprintf(err, n, "ewald_beta must be >= 0"); return TKHP_EINVAL; }
@@ -32,7 +32,7 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
         snprintf(err, n, "ewald_beta * cutoff must be <= 6 (range of the erfc fits)");
         return TKHP_EINVAL;
     }
-    if (p->precision == TKHP_MIXED && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }
+    if (p->precision != TKHP_FP64 && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED / FIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }
     if (p->max_tiles_per_block < 0 || p->max_nbrs_per_cluster < 0 || p->max_nbrs_per_atom < 0) { snprintf(err, n, "negative capacity"); return TKHP_EINVAL; }
     if (p->solver_flags & ~(TKHP_SOLVER_NO_PERSISTENT | TKHP_SOLVER_NO_FUSED_STEP) || p->reserved != 0) { snprintf(err, n, "unknown solver_flags / non-zero reserved field"); return TKHP_EINVAL; }
     if (p->max_stage_per_chunk < 0 || (p->max_stage_per_chunk & 31)) { snprintf(err, n, "max_stage_per_chunk must be a non-negative multiple of 32"); return TKHP_EINVAL; }
@@ -210,6 +210,7 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     if (cudaGetDeviceProperties(&prop, params->device) != cudaSuccess) { delete c; return TKHP_ECUDA; }
     c->sm_count = prop.multiProcessorCount;
     atom_far_setup(c);
+    c->fixed = params->precision == TKHP_FIXED;
     c->no_persist = (params->solver_flags & TKHP_SOLVER_NO_PERSISTENT) != 0;
     c->no_fused_step = (params->solver_flags & TKHP_SOLVER_NO_FUSED_STEP) != 0;
     if (cluster_pairs_configure(c) || atom_lists_configure(c) || atom_pairs_configure(c) || atom_solve_configure(c)) {

@@ -49,8 +49,8 @@ struct PcgFuse {
 template <typename real>
 struct Partial {
     real x = 0, y = 0, z = 0;
-    __device__ __forceinline__ void flush(double &dx, double &dy, double &dz) {
-        dx += (double)x; dy += (double)y; dz += (double)z;
+    __device__ __forceinline__ void flush(double &dx, double &dy, double &dz, bool fixed) {
+        acc_add(dx, x, fixed); acc_add(dy, y, fixed); acc_add(dz, z, fixed);
         x = 0; y = 0; z = 0;
     }
 };
@@ -213,6 +213,7 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     double dx = 0.0, dy = 0.0, dz = 0.0;
     Partial<real> A;
     int since_flush = 0;
+    const bool fixed = sizeof(real) == 4 && kc.fixed != 0;
 
     if (t < N_DUMMY) {                         // permanent dummy records: far away, zero payload
         vec4 far, zero;
@@ -279,8 +280,8 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
                             eval_pairs<real, MODE, 2>(s_base, pay_stride, o2, pi, gi, kc, A);
                         }
                     }
-                    if (++since_flush == 4) {          // every 32 entries: FP32 partial -> FP64 accumulator
-                        A.flush(dx, dy, dz);
+                    if (++since_flush == 4) {          // every 32 entries: FP32 partial -> 64-bit container
+                        A.flush(dx, dy, dz, fixed);
                         since_flush = 0;
                     }
                 }
@@ -288,7 +289,8 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             sd = seg[++d];
         }
     }
-    A.flush(dx, dy, dz);
+    A.flush(dx, dy, dz, fixed);
+    dx = acc_value(dx, fixed); dy = acc_value(dy, fixed); dz = acc_value(dz, fixed);
     pair_epilogue<MODE == MODE_TMU>(smem_raw, dx, dy, dz, wpb, part, active, slot, n_pad, acc, st, fuse);
 }
 
@@ -387,7 +389,8 @@ k_atom_tmu32(ClusterWs ws, const float4 *__restrict__ gpos, const float4 *__rest
 #endif
         tmu_walk<FAR>(seg, c, d, sd, tg, wpb, R, S, L, K, A, n_rows, dx, dy, dz);
     }
-    A.flush(dx, dy, dz);
+    A.flush(dx, dy, dz, K.fixed);
+    dx = acc_value(dx, K.fixed != 0); dy = acc_value(dy, K.fixed != 0); dz = acc_value(dz, K.fixed != 0);
     pair_epilogue<true>(smem_raw, dx, dy, dz, wpb, part, active, slot, n_pad, acc, st, fuse);
 }
 
@@ -402,7 +405,7 @@ void atom_far_setup(Ctx *c) {
     c->far_x0 = 0.0;
     c->far_rmin = 0.0;
     for (int k = 0; k < 6; ++k) c->far_q[k] = 0.f;
-    if (c->p.precision != TKHP_MIXED || !(beta > 0.0) || z_max < 1.25 * z_min) return;    // no far class: full formula everywhere
+    if (c->p.precision == TKHP_FP64 || !(beta > 0.0) || z_max < 1.25 * z_min) return;    // no far class: full formula everywhere
     c->far_on = true;
     constexpr int D = 5;
     const double a = 1.0 / z_max, b = 1.0 / z_min;
@@ -443,6 +446,7 @@ static int launch_atom_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     k.box = (real)1;
     k.inv_box = (real)0;
     k.pb = k.nb2l = k.c1b = k.k3 = (real)0;
+    k.fixed = c->fixed ? 1 : 0;
     PcgFuse fuse;
     fuse.on = MODE == MODE_TMU && c->fuse_q;
     fuse.self = 4.0 * c->p.ewald_beta * c->p.ewald_beta * c->p.ewald_beta / (3.0 * SQRT_PI);
@@ -468,6 +472,7 @@ static int launch_tmu32(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     K.c1b = (float)(2.0 / SQRT_PI * b);
     K.k3 = (float)(4.0 / (3.0 * SQRT_PI) * b * b * b);
     for (int k = 0; k < 6; ++k) K.q[k] = c->far_q[k];
+    K.fixed = c->fixed ? 1 : 0;
     PcgFuse fuse;
     fuse.on = c->fuse_q;
     fuse.self = 4.0 * b * b * b / (3.0 * SQRT_PI);
@@ -502,12 +507,12 @@ int atom_pairs_configure(Ctx *c) {
 
 int atom_tmatvec(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
-    return c->p.precision == TKHP_MIXED ? launch_tmu32(c, ws, s) : launch_atom_pairs<double, MODE_TMU>(c, ws, s);
+    return c->p.precision != TKHP_FP64 ? launch_tmu32(c, ws, s) : launch_atom_pairs<double, MODE_TMU>(c, ws, s);
 }
 
 int atom_field(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
-    return c->p.precision == TKHP_MIXED ? launch_atom_pairs<float, MODE_FIELD>(c, ws, s)
+    return c->p.precision != TKHP_FP64 ? launch_atom_pairs<float, MODE_FIELD>(c, ws, s)
                                         : launch_atom_pairs<double, MODE_FIELD>(c, ws, s);
 }
 

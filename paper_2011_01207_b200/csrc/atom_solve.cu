@@ -205,7 +205,8 @@ k_pcg_persist(SolveArgs a) {
             int d = 0, n_rows = 0, tg = part;
             int2 sd = seg[0];
             tmu_walk<FAR>(seg, 0, d, sd, tg, wpb, R, S, L, a.K, A, n_rows, dx, dy, dz);
-            A.flush(dx, dy, dz);
+            A.flush(dx, dy, dz, a.K.fixed);
+            dx = acc_value(dx, a.K.fixed); dy = acc_value(dy, a.K.fixed); dz = acc_value(dz, a.K.fixed);
         }
         if (SPLIT && wpb > 1) {                    // uniform over the CTA: add the parts of a block, part 1 first
             __syncthreads();
@@ -329,7 +330,7 @@ int atom_solve_configure(Ctx *c) {
 
 // Can the persistent kernel run this solve?  (list header on the host: ensure_header has run)
 bool atom_solve_eligible(Ctx *c) {
-    if (!c->coop_ok || c->no_persist || c->p.precision != TKHP_MIXED || c->list_mode_in_use != TKHP_LIST_ATOM) return false;
+    if (!c->coop_ok || c->no_persist || c->p.precision == TKHP_FP64 || c->list_mode_in_use != TKHP_LIST_ATOM) return false;
     ClusterWs ws = get_ws(c);
     const int s_max = atom_chunk_capacity(false, ws.chunk_cap);
     const int need = c->h_state->max_stage;
@@ -361,6 +362,7 @@ int atom_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess
     a.K.c1b = (float)(2.0 / SQRT_PI * b);
     a.K.k3 = (float)(4.0 / (3.0 * SQRT_PI) * b * b * b);
     for (int k = 0; k < 6; ++k) a.K.q[k] = c->far_q[k];
+    a.K.fixed = c->fixed ? 1 : 0;
     a.field = d_field;
     a.mu = d_mu;
     a.perm = c->perm;

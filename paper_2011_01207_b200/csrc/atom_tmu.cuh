@@ -14,10 +14,11 @@ namespace tkhp {
 struct PartialTmu {
     f2 cxy = 0ull, mxy = 0ull;
     float cz = 0.f, mz = 0.f;
-    __device__ __forceinline__ void flush(double &dx, double &dy, double &dz) {
-        dx += (double)fmaf(3.0f, lo(cxy), -lo(mxy));
-        dy += (double)fmaf(3.0f, hi(cxy), -hi(mxy));
-        dz += (double)fmaf(3.0f, cz, -mz);
+    // into the 64-bit containers: FP64, or int64 fixed point (TKHP_FIXED, common.cuh acc_add)
+    __device__ __forceinline__ void flush(double &dx, double &dy, double &dz, int fixed) {
+        acc_add(dx, fmaf(3.0f, lo(cxy), -lo(mxy)), fixed != 0);
+        acc_add(dy, fmaf(3.0f, hi(cxy), -hi(mxy)), fixed != 0);
+        acc_add(dz, fmaf(3.0f, cz, -mz), fixed != 0);
         cxy = 0ull; mxy = 0ull; cz = 0.f; mz = 0.f;
     }
 };
@@ -38,6 +39,7 @@ struct TmuConsts {
     float c1b;      // (2/sqrt pi) beta:      c z = c1b R
     float k3;       // (4/(3 sqrt pi)) beta^3: (2c/3) z^3 = k3 R^3
     float q[6];     // far fit: erfcx(beta R) = t (q0 + q1 t + ... + q5 t^5), t = 1/R
+    int fixed;      // TKHP_FIXED: the 64-bit accumulators are int64 with 34 fractional bits
 };
 struct TmuSmem {
     const unsigned char *a, *b, *w;   // generic pointers into shared memory
@@ -203,7 +205,7 @@ __device__ __forceinline__ void tmu_walk(const int2 *__restrict__ seg, int c, in
         for (; tg < f_full; tg += wpb) {
             const uint4 e = R.next();
             tmu_row<FAR>(S, e, 4, L, K, A);
-            if ((++n_rows & 3) == 0) A.flush(dx, dy, dz);   // every 32 entries: FP32 partial -> FP64
+            if ((++n_rows & 3) == 0) A.flush(dx, dy, dz, K.fixed);   // every 32 entries: FP32 partial -> 64-bit container
         }
         if ((ncf & 3) && tg == f_full) {
             const uint4 e = R.next();
@@ -214,7 +216,7 @@ __device__ __forceinline__ void tmu_walk(const int2 *__restrict__ seg, int c, in
         for (; tg < n_full; tg += wpb) {
             const uint4 e = R.next();
             tmu_row<false>(S, e, 4, L, K, A);
-            if ((++n_rows & 3) == 0) A.flush(dx, dy, dz);
+            if ((++n_rows & 3) == 0) A.flush(dx, dy, dz, K.fixed);
         }
         if ((ncn & 3) && tg == n_full) {
             const uint4 e = R.next();

@@ -55,6 +55,7 @@ k_cluster_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos
     double dx = 0.0, dy = 0.0, dz = 0.0;
     real ax = 0, ay = 0, az = 0;
     int since_flush = 0;
+    const bool fixed = sizeof(real) == 4 && kc.fixed != 0;
     unsigned e = ql < L ? (unsigned)ent[ql] : 0xffffffffu;     // entries [cur, cur+8) of this cluster
 
     if (t == 0) {                              // permanent dummy record: far away, zero payload
@@ -138,18 +139,18 @@ k_cluster_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos
                 }
             }
             e = e_next;
-            if (++since_flush == 4) {          // every 32 entries: FP32 partial -> FP64 accumulator
-                dx += (double)ax; dy += (double)ay; dz += (double)az;
+            if (++since_flush == 4) {          // every 32 entries: FP32 partial -> 64-bit container
+                acc_add(dx, ax, fixed); acc_add(dy, ay, fixed); acc_add(dz, az, fixed);
                 ax = 0; ay = 0; az = 0;
                 since_flush = 0;
             }
         }
     }
     if (!active) return;
-    dx += (double)ax; dy += (double)ay; dz += (double)az;
-    acc[slot] = dx;
-    acc[n_pad + slot] = dy;
-    acc[2 * (size_t)n_pad + slot] = dz;
+    acc_add(dx, ax, fixed); acc_add(dy, ay, fixed); acc_add(dz, az, fixed);
+    acc[slot] = acc_value(dx, fixed);
+    acc[n_pad + slot] = acc_value(dy, fixed);
+    acc[2 * (size_t)n_pad + slot] = acc_value(dz, fixed);
 }
 
 template <typename real, int MODE>
@@ -170,6 +171,7 @@ static int launch_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     k.rc2 = (real)(c->p.cutoff * c->p.cutoff);
     k.box = (real)1;
     k.inv_box = (real)0;
+    k.fixed = c->fixed ? 1 : 0;
     const vec4 *gpos = which ? (const vec4 *)ws.gpos64 : (const vec4 *)ws.gpos32;
     const vec4 *spos = which ? (const vec4 *)ws.stage_pos64 : (const vec4 *)ws.stage_pos32;
     const vec4 *data;
@@ -192,13 +194,13 @@ int cluster_pairs_configure(Ctx *c) {
 
 int cluster_tmatvec(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
-    return c->p.precision == TKHP_MIXED ? launch_pairs<float, MODE_TMU>(c, ws, s)
+    return c->p.precision != TKHP_FP64 ? launch_pairs<float, MODE_TMU>(c, ws, s)
                                         : launch_pairs<double, MODE_TMU>(c, ws, s);
 }
 
 int cluster_field(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
-    return c->p.precision == TKHP_MIXED ? launch_pairs<float, MODE_FIELD>(c, ws, s)
+    return c->p.precision != TKHP_FP64 ? launch_pairs<float, MODE_FIELD>(c, ws, s)
                                         : launch_pairs<double, MODE_FIELD>(c, ws, s);
 }
 

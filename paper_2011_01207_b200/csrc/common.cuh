@@ -54,6 +54,7 @@ struct DeviceState {
     double pq, rr, gamma, delta;
     unsigned ticket;        // last-block reductions (reduce.cuh); 0 between kernels
     int bar_gen;            // grid barrier of k_pcg_step: the iteration whose partial sums are complete
+    unsigned long long energy_fixed;   // TKHP_FIXED: int64 container of the energy (30 fractional bits), 0 between kernels
     unsigned bar_count;     // grid barrier of k_pcg_persist: arrivals (monotonic within a solve) ...
     unsigned bar_release;   // ... and the last barrier every CTA has reached (adjacent: zeroed together)
     int conv_at;            // PCG: iterations with index >= conv_at are skipped on the device
@@ -117,6 +118,7 @@ struct Ctx {
     double far_rmin;
     float far_q[6];         // far fit of erfcx in t = 1/R
     float4 *u32;            // n_pad: operand exchange of the persistent PCG kernel (atom_solve.cu)
+    bool fixed;             // TKHP_FIXED: int64 fixed-point accumulators in the FP32 pair kernels and the energy
     bool coop_ok;           // the device supports cooperative launches
     bool no_persist, no_fused_step;   // tkhp_params.solver_flags
     bool fuse_q;            // ATOM-mode T.mu kernel also forms q = p/alpha - T p - self p and p.q (PCG)
@@ -218,6 +220,21 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
                    int *h_iters, double *h_rms, cudaStream_t s);
 int do_polar_energy(Ctx *c, const double *d_mu, const double *d_field, double *d_energy, cudaStream_t s);
 int ensure_header(Ctx *c, cudaStream_t s);          // list header on the host (one small sync per build)
+
+// ---- fixed-point containers (TKHP_FIXED; eqs 2-3): a = int(round(x 2^fB)), x = real(a) / 2^fB.
+// A 64-bit accumulator register is declared double in the kernels; in FIXED mode it carries the BITS
+// of the int64 container (0.0 is integer 0), so that one kernel serves both modes.
+constexpr int FIX_VEC_BITS = 34;      // field and T.mu accumulators
+constexpr int FIX_ENERGY_BITS = 30;   // energy
+__device__ __forceinline__ long long to_fixed(float x, int fb) { return __float2ll_rn(x * (float)(1ll << fb)); }
+__device__ __forceinline__ void acc_add(double &a, float x, bool fixed) {
+    if (fixed) a = __longlong_as_double(__double_as_longlong(a) + to_fixed(x, FIX_VEC_BITS));
+    else a += (double)x;
+}
+__device__ __forceinline__ void acc_add(double &a, double x, bool) { a += x; }     // FP64 mode
+__device__ __forceinline__ double acc_value(double a, bool fixed) {
+    return fixed ? (double)__double_as_longlong(a) * (1.0 / (double)(1ll << FIX_VEC_BITS)) : a;
+}
 
 // warp helpers
 __device__ __forceinline__ double warp_min(double v) {

@@ -56,7 +56,7 @@ static int run_peak(int device, double seconds, double *tflops) {
 
 extern "C" int tkhp_fma_peak(int32_t device, int32_t precision, double seconds, double *tflops) {
     if (!tflops || seconds <= 0.0) return TKHP_EINVAL;
-    if (precision == TKHP_MIXED) return tkhp::run_peak<float>(device, seconds, tflops);
+    if (precision == TKHP_MIXED || precision == TKHP_FIXED) return tkhp::run_peak<float>(device, seconds, tflops);
     if (precision == TKHP_FP64) return tkhp::run_peak<double>(device, seconds, tflops);
     return TKHP_EINVAL;
 }

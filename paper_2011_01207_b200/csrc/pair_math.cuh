@@ -38,6 +38,7 @@ struct PairConsts {
     real nb2l;      // -beta^2 log2 e:          e^{-z^2} = ex2(nb2l R^2)
     real c1b;       // (2/sqrt pi) beta:        c z = c1b R
     real k3;        // (4/(3 sqrt pi)) beta^3:  (2c/3) z^3 = k3 R^3
+    int fixed;      // TKHP_FIXED (FP32 kernels only): int64 fixed-point accumulators (common.cuh acc_add)
 };
 
 template <typename real> struct Vec4;

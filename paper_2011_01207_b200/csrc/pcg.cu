@@ -317,6 +317,32 @@ k_energy(const double *__restrict__ mu, const double *__restrict__ field, long l
     if (grid_sum2_last_block(part, &st->ticket, s, dmy) && threadIdx.x == 0) *energy = -0.5 * COULOMB * s;
 }
 
+// TKHP_FIXED: every term -1/2 f mu_i.E_i goes into an int64 container with 30 fractional
+// bits (kcal/mol); integer sums do not depend on the order, so warp sums and one integer atomic per
+// warp are deterministic.  The last block converts back (eq. 3) and clears the container.
+__global__ void __launch_bounds__(RED_THREADS)
+k_energy_fixed(const double *__restrict__ mu, const double *__restrict__ field, long long n3, DeviceState *st,
+               double *__restrict__ energy) {
+    long long s = 0;
+    const double scale = -0.5 * COULOMB * (double)(1ll << FIX_ENERGY_BITS);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += (long long)gridDim.x * blockDim.x)
+        s += __double2ll_rn(mu[i] * field[i] * scale);
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(&st->energy_fixed, (unsigned long long)s);
+    __shared__ bool s_last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = atomicInc(&st->ticket, gridDim.x - 1) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence();
+        const long long tot = (long long)atomicExch(&st->energy_fixed, 0ull);
+        *energy = (double)tot * (1.0 / (double)(1ll << FIX_ENERGY_BITS));
+    }
+}
+
 // ----------------------------------------------------------------------------- host drivers
 static inline double self_coeff(const tkhp_params &p) {
     const double b = p.ewald_beta;
@@ -365,7 +391,7 @@ int run_field(Ctx *c, cudaStream_t s) {
 int do_perm_field(Ctx *c, const double *d_q, const double *d_dip, const double *d_quad, double *d_field,
                   cudaStream_t s) {
     const int g = div_up(c->n_pad, VEC_THREADS);
-    if (c->p.precision == TKHP_MIXED)
+    if (c->p.precision != TKHP_FP64)
         k_pack_multipoles<float4><<<g, VEC_THREADS, 0, s>>>(d_q, d_dip, d_quad, c->group_o, c->perm, c->n_pad, c->mp32);
     else
         k_pack_multipoles<double4><<<g, VEC_THREADS, 0, s>>>(d_q, d_dip, d_quad, c->group_o, c->perm, c->n_pad, c->mp64);
@@ -381,7 +407,7 @@ int do_perm_field(Ctx *c, const double *d_q, const double *d_dip, const double *
 
 int do_tmatvec(Ctx *c, const double *d_mu, double *d_out, cudaStream_t s) {
     const int g = div_up(c->n_pad, VEC_THREADS);
-    if (c->p.precision == TKHP_MIXED)
+    if (c->p.precision != TKHP_FP64)
         k_pack_mu_user<float4><<<g, VEC_THREADS, 0, s>>>(d_mu, c->perm, c->n_pad, c->mu32);
     else
         k_pack_mu_user<double4><<<g, VEC_THREADS, 0, s>>>(d_mu, c->perm, c->n_pad, c->mu64);
@@ -423,7 +449,7 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
     const int g1 = div_up(n_pad, VEC_THREADS);
     const int gv = vec_grid(c);
     const double self = self_coeff(c->p);
-    const bool mixed = c->p.precision == TKHP_MIXED;
+    const bool mixed = c->p.precision != TKHP_FP64;
     double *part_rz = c->partials;
     double *part_pq = c->partials + 2 * (size_t)c->part_cap;
     const bool fused_q = c->list_mode_in_use == TKHP_LIST_ATOM;   // q and p.q in the pair kernel's epilogue
@@ -553,7 +579,8 @@ int do_polar_energy(Ctx *c, const double *d_mu, const double *d_field, double *d
     int g = div_up(n3, VEC_THREADS);
     if (g > MAX_PARTIALS) g = MAX_PARTIALS;
     double *part = c->partials + 4 * (size_t)c->part_cap;
-    k_energy<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, part, c->st, d_energy);
+    if (c->fixed) k_energy_fixed<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, c->st, d_energy);
+    else k_energy<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, part, c->st, d_energy);
     c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;

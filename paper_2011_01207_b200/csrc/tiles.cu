@@ -48,6 +48,15 @@ __device__ __forceinline__ void wrap_pair(real &Rx, real &Ry, real &Rz, const Pa
     }
 }
 
+// a tile's contribution into the 64-bit accumulator of an atom: an FP64 atomic, or (TKHP_FIXED) an
+// integer atomic on the int64 fixed-point container -- "we adopt a 64 bits container" with "atomic
+// operations": the integer sum does not depend on the order of the tiles
+template <typename real>
+__device__ __forceinline__ void acc_atomic(double *p, real v, bool fixed) {
+    if (fixed) atomicAdd(reinterpret_cast<unsigned long long *>(p), (unsigned long long)to_fixed((float)v, FIX_VEC_BITS));
+    else atomicAdd(p, (double)v);
+}
+
 // ----------------------------------------------------------------------------- T.mu
 template <typename real, bool PPI>
 __global__ void __launch_bounds__(TILE_WARPS * 32)
@@ -60,6 +69,7 @@ k_tiles_tmu(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st,
     __shared__ vec4 s_mu[TILE_WARPS][BLOCK];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
+    const bool fixed = sizeof(real) == 4 && kc.fixed != 0;
     const long long n_tiles = st->n_tiles;
     const long long stride = (long long)gridDim.x * TILE_WARPS;
     for (long long t = (long long)blockIdx.x * TILE_WARPS + w; t < n_tiles; t += stride) {
@@ -96,9 +106,9 @@ k_tiles_tmu(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st,
                 bx = shfl_real(bx, src); by = shfl_real(by, src); bz = shfl_real(bz, src);
             }
             const int sj = J * BLOCK + lane;
-            atomicAdd(&acc[sj], (double)bx);
-            atomicAdd(&acc[n_pad + sj], (double)by);
-            atomicAdd(&acc[2 * n_pad + sj], (double)bz);
+            acc_atomic(&acc[sj], bx, fixed);
+            acc_atomic(&acc[n_pad + sj], by, fixed);
+            acc_atomic(&acc[2 * n_pad + sj], bz, fixed);
         } else {
             // diagonal tile: every ordered pair i <- j, j != i (no mirror update)
 #pragma unroll 4
@@ -118,9 +128,9 @@ k_tiles_tmu(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st,
             }
         }
         const int si = I * BLOCK + lane;
-        atomicAdd(&acc[si], (double)ax);
-        atomicAdd(&acc[n_pad + si], (double)ay);
-        atomicAdd(&acc[2 * n_pad + si], (double)az);
+        acc_atomic(&acc[si], ax, fixed);
+        acc_atomic(&acc[n_pad + si], ay, fixed);
+        acc_atomic(&acc[2 * n_pad + si], az, fixed);
     }
 }
 
@@ -138,6 +148,7 @@ k_tiles_field(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st
     __shared__ vec4 s_mp[3][TILE_WARPS][BLOCK];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
+    const bool fixed = sizeof(real) == 4 && kc.fixed != 0;
     const long long n_tiles = st->n_tiles;
     const long long stride = (long long)gridDim.x * TILE_WARPS;
     for (long long t = (long long)blockIdx.x * TILE_WARPS + w; t < n_tiles; t += stride) {
@@ -183,14 +194,21 @@ k_tiles_field(const int2 *__restrict__ pairs, const DeviceState *__restrict__ st
             }
         }
         if (!diag) {
-            atomicAdd(&acc[sj], (double)bx);
-            atomicAdd(&acc[n_pad + sj], (double)by);
-            atomicAdd(&acc[2 * n_pad + sj], (double)bz);
+            acc_atomic(&acc[sj], bx, fixed);
+            acc_atomic(&acc[n_pad + sj], by, fixed);
+            acc_atomic(&acc[2 * n_pad + sj], bz, fixed);
         }
-        atomicAdd(&acc[si], (double)ax);
-        atomicAdd(&acc[n_pad + si], (double)ay);
-        atomicAdd(&acc[2 * n_pad + si], (double)az);
+        acc_atomic(&acc[si], ax, fixed);
+        acc_atomic(&acc[n_pad + si], ay, fixed);
+        acc_atomic(&acc[2 * n_pad + si], az, fixed);
     }
+}
+
+// TKHP_FIXED: the tile kernels have added int64 fixed-point values into `acc` with integer atomics (the
+// paper's FP mode: deterministic whatever the order); back to FP64 values in place
+__global__ void k_fixed_to_double(double *__restrict__ acc, size_t n) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) acc[i] = acc_value(acc[i], true);
 }
 
 template <typename real>
@@ -202,6 +220,7 @@ static PairConsts<real> make_consts(const tkhp_params &p) {
     k.rc2 = (real)(p.cutoff * p.cutoff);
     k.box = (real)(p.box > 0.0 ? p.box : 1.0);
     k.inv_box = (real)(p.box > 0.0 ? 1.0 / p.box : 0.0);
+    k.fixed = (sizeof(real) == 4 && p.precision == TKHP_FIXED) ? 1 : 0;
     return k;
 }
 
@@ -228,11 +247,16 @@ static int tile_grid(Ctx *c) {
 int tiles_tmatvec(Ctx *c, cudaStream_t s) {
     const int grid = tile_grid(c);
     const tkhp_params &p = c->p;
-    if (p.precision == TKHP_MIXED)
+    if (p.precision != TKHP_FP64)
         TKHP_LAUNCH_TILES(k_tiles_tmu, float, c->xyzw32, c->mu32);
     else
         TKHP_LAUNCH_TILES(k_tiles_tmu, double, c->xyzw64, c->mu64);
     c->n_launches += 1;
+    if (c->fixed) {
+        const size_t n3 = 3 * (size_t)c->n_pad;
+        k_fixed_to_double<<<(unsigned)((n3 + 255) / 256), 256, 0, s>>>(c->acc, n3);
+        c->n_launches += 1;
+    }
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }
@@ -240,11 +264,16 @@ int tiles_tmatvec(Ctx *c, cudaStream_t s) {
 int tiles_field(Ctx *c, cudaStream_t s) {
     const int grid = tile_grid(c);
     const tkhp_params &p = c->p;
-    if (p.precision == TKHP_MIXED)
+    if (p.precision != TKHP_FP64)
         TKHP_LAUNCH_TILES(k_tiles_field, float, c->xyzw32, c->mp32);
     else
         TKHP_LAUNCH_TILES(k_tiles_field, double, c->xyzw64, c->mp64);
     c->n_launches += 1;
+    if (c->fixed) {
+        const size_t n3 = 3 * (size_t)c->n_pad;
+        k_fixed_to_double<<<(unsigned)((n3 + 255) / 256), 256, 0, s>>>(c->acc, n3);
+        c->n_launches += 1;
+    }
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }

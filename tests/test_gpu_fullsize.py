@@ -269,3 +269,22 @@ def test_cfg4_cutoff_sweep(cutoff, precision):
     _, it6, rms6 = P.polar_solve(Eg, tol=1e-6)
     assert rms6 < 1e-6 and 6 <= it6 <= 14                      # 9-10 iterations at 9-12 A
     P.close()
+
+
+def test_cfg2_fixed_point_mode(cfg2, cfg2_oracle):
+    """Config 2 in the paper's FP mode (TKHP_FIXED): every row against the oracle at the
+    MIXED bars, through the persistent solve kernel."""
+    import paper_2011_01207_b200 as pk
+    s, ref = cfg2, cfg2_oracle
+    P = pk.Polarizer.for_system(s, precision=pk.TKHP_FIXED, list_mode=pk.TKHP_LIST_ATOM)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    assert P.nblist_stats(count_pairs=False)[2] == pk.TKHP_LIST_ATOM
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    _assert_close(Eg.cpu().numpy(), ref["E"], 1e-5)
+    _assert_close(P.tmatvec(ref["probe"]).cpu().numpy(), ref["T"], 1e-5)
+    mu_g, it, rms = P.polar_solve(Eg, tol=1e-8)
+    assert rms < 1e-8
+    _assert_close(mu_g.cpu().numpy(), ref["mu"], 1e-5)
+    e_g = float(P.polar_energy(mu_g, Eg).cpu())
+    assert abs(e_g - ref["e_pol"]) <= 1e-6 * abs(ref["e_pol"])
+    P.close()

@@ -402,3 +402,63 @@ def test_open_boundary_elongated_system():
         assert P.nblist_stats()[0] == oracle.count_pairs(s)
         _assert_close(P.perm_field(s.charge, s.dipole, s.quad).cpu().numpy(), oracle.perm_field(s), TOL_VEC[precision])
         P.close()
+
+
+# ------------------------------------------------------------------ TKHP_FIXED: the paper's FP mode
+@pytest.mark.parametrize("list_mode", ["tiles", "cluster", "atom"])
+@pytest.mark.parametrize("name", ["cfg0", "water_6000"])
+def test_fixed_point_mode_matches_the_oracle(name, list_mode):
+    """TKHP_FIXED (eqs 2-3): FP32 pair math, int64 containers with 34 fractional bits for the
+    field and T.mu accumulators and 30 for the energy.  Same bars as MIXED (BASELINE.json), bit-identical
+    repeats (in TILES mode too, where the containers are filled by integer atomics in any order), and the
+    energy is an integer multiple of 2^-30 kcal/mol."""
+    pk = _pk()
+    s = SYSTEMS[name]()
+    P = pk.Polarizer.for_system(s, precision=pk.TKHP_FIXED,
+                                list_mode={"tiles": pk.TKHP_LIST_TILES, "cluster": pk.TKHP_LIST_CLUSTER, "atom": pk.TKHP_LIST_ATOM}[list_mode])
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    E_ref = oracle.perm_field(s)
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    _assert_close(Eg.cpu().numpy(), E_ref, 1e-5)
+    rng = np.random.default_rng(12)
+    mu = rng.standard_normal((s.n_atoms, 3)) * 0.1
+    t1 = P.tmatvec(mu).cpu().numpy()
+    _assert_close(t1, oracle.tmatvec(s, mu), 1e-5)
+    for _ in range(3):
+        assert np.array_equal(P.tmatvec(mu).cpu().numpy(), t1)
+        assert np.array_equal(P.perm_field(s.charge, s.dipole, s.quad).cpu().numpy(), Eg.cpu().numpy())
+    mu_ref = oracle.dense_solve(s, E_ref)
+    mu_g, it, rms = P.polar_solve(Eg, tol=1e-8)
+    assert rms < 1e-8
+    _assert_close(mu_g.cpu().numpy(), mu_ref, 1e-5)
+    e_ref = oracle.polar_energy(mu_ref, E_ref)
+    e_g = float(P.polar_energy(mu_g, Eg).cpu())
+    assert abs(e_g - e_ref) <= 1e-6 * abs(e_ref)
+    scaled = e_g * float(1 << oracle.FIX_ENERGY_BITS)
+    assert scaled == np.rint(scaled) and int(oracle.to_fixed(e_g, oracle.FIX_ENERGY_BITS)) == int(scaled)
+    P.close()
+
+
+@pytest.mark.parametrize("list_mode", ["tiles", "atom"])
+def test_fixed_point_accumulators_hold_multiples_of_2_to_minus_34(list_mode):
+    """Open boundary, beta = 0 (no self term), one atom per group (no mask correction): the library's
+    T.mu output IS the accumulator, so every component must be an integer multiple of 2^-34 (eq. 3)."""
+    pk = _pk()
+    s = tiny_cluster(200, 31, box=0.0, spread=14.0, group_size=1, cutoff=6.0, skin=1.0)
+    P = pk.Polarizer.for_system(s, precision=pk.TKHP_FIXED,
+                                list_mode=pk.TKHP_LIST_TILES if list_mode == "tiles" else pk.TKHP_LIST_ATOM)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    rng = np.random.default_rng(13)
+    mu = rng.standard_normal((s.n_atoms, 3)) * 0.1
+    out = P.tmatvec(mu).cpu().numpy()
+    _assert_close(out, oracle.tmatvec(s, mu), 1e-5)
+    a = oracle.to_fixed(out, oracle.FIX_VEC_BITS)
+    assert np.array_equal(oracle.from_fixed(a, oracle.FIX_VEC_BITS), out)
+    assert np.abs(out).max() > 1e-3                              # (not trivially zero)
+    # MIXED on the same system is NOT confined to that grid
+    Pm = pk.Polarizer.for_system(s, precision=pk.TKHP_MIXED,
+                                 list_mode=pk.TKHP_LIST_TILES if list_mode == "tiles" else pk.TKHP_LIST_ATOM)
+    Pm.nblist_build(s.pos, s.polarizability, s.group_id)
+    om = Pm.tmatvec(mu).cpu().numpy()
+    assert not np.array_equal(oracle.from_fixed(oracle.to_fixed(om, oracle.FIX_VEC_BITS), oracle.FIX_VEC_BITS), om)
+    P.close(); Pm.close()

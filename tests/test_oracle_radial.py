@@ -127,3 +127,26 @@ def test_G_is_iterated_derivative_of_one_kernel(s, R):
     want = [float(g1(mp.mpf(R))), float(g2(mp.mpf(R))), float(g3(mp.mpf(R)))]
     got = oracle.pair_G(beta, a, ai, aj, s, R)
     np.testing.assert_allclose(got, want, rtol=2e-9, atol=1e-16)
+
+
+def test_fixed_point_containers_eqs_2_and_3():
+    """Paper eqs (2)-(3): a = int(round(x 2^fB)), x = real(a) / 2^fB, with the paper's
+    numbers: 34 fractional bits for vectors leave 30 for the integer part ("absolute limit 2^29"),
+    30 fractional bits for the energy, and "27 bits ... capture 8 digits after the decimal point"."""
+    import oracle as o
+    assert o.FIX_VEC_BITS == 34 and o.FIX_ENERGY_BITS == 30
+    assert int(o.to_fixed(1.0, 34)) == 1 << 34 and int(o.to_fixed(-0.5, 30)) == -(1 << 29)
+    assert float(o.from_fixed(1 << 34, 34)) == 1.0
+    # the container holds |x| < 2^29 with 34 fractional bits (63 value bits)
+    assert int(o.to_fixed(2.0 ** 29 - 1.0, 34)) < 2 ** 63
+    # resolution: half a unit in the last place of the container
+    rng = np.random.default_rng(3)
+    x = rng.uniform(-100.0, 100.0, 1000)
+    for fb in (27, 30, 34):
+        back = o.from_fixed(o.to_fixed(x, fb), fb)
+        assert np.max(np.abs(back - x)) <= 2.0 ** -(fb + 1)
+        assert np.all(o.to_fixed(back, fb) == o.to_fixed(x, fb))          # idempotent
+    assert 2.0 ** -27 < 1e-8 < 2.0 ** -26                                  # 27 bits <-> 8 decimal digits
+    # integer sums are order independent (what makes the mode deterministic)
+    a = o.to_fixed(rng.standard_normal(4096) * 1e-3, 34)
+    assert int(a.sum()) == int(a[::-1].sum()) == int(np.sort(a).sum())
