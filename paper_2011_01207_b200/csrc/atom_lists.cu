@@ -93,9 +93,13 @@ __device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16
     }
 }
 
-// ---- pass 1: scan.  One CTA per group, one warp per block, one lane per atom.  FAR hits go straight
-// to the block's rows in arrival order (pass 2 permutes them in place), NEAR hits wait in a small
-// shared-memory buffer until the length of the far part of the segment is known.
+// ---- pass 1: scan.  One CTA per group, one warp per block, one lane per atom.  The kernel is bound by
+// its instruction count, so the appends are branch-free: a hit is written (predicated) into a small
+// per-lane queue in shared memory -- FAR hits into a 16-entry ring from which every lane writes its
+// own 16-byte row (8 entries, arrival order; pass 2 permutes them in place) as soon as it has one,
+// NEAR hits into a buffer that waits until the length of the far part of the segment is known.
+constexpr int FQ = 16;                  // entries of a lane's far ring
+
 template <typename real>
 __global__ void __launch_bounds__(GT)
 k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
@@ -103,7 +107,7 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             int s_chunk, DeviceState *st) {
     using vec4 = typename Vec4<real>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk] | near buffers [GB][NEAR_CAP][32] u16
+    vec4 *s_pos = reinterpret_cast<vec4 *>(smem_raw);          // [s_chunk] | per warp: near buffer [NEAR_CAP][32], far ring [FQ][32] (u16)
 
     const int g = blockIdx.x, t = threadIdx.x, lane = t & 31, w = t >> 5;
     const int b0 = ws.group_first[g], nb = ws.group_first[g + 1] - b0;
@@ -113,8 +117,7 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const bool active = w < nb;
     const int blk = b0 + (active ? w : 0);
     int2 *__restrict__ seg = ws.aseg + (size_t)blk * NSEG_MAX;
-    // padding entries point at the record after the largest chunk of THIS group (the kernels put a
-    // far-away record with zero payload there)
+    // padding entries point at the (first) dummy record after the largest chunk of THIS group
     const unsigned dummy = (unsigned)atom_dummy_index(count, n_chunks) * (unsigned)sizeof(vec4);
     if (n_chunks > NCH_MAX) {                      // uniform over the CTA
         if (t == 0) st->atom_bad = 1;
@@ -128,23 +131,27 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const int L = active ? ws.oct_len[oct] : 0;
     const uint4 *__restrict__ ent8 = reinterpret_cast<const uint4 *>(ws.entries + (size_t)oct * ws.l_cap);  // 8 entries per load
     const int L8 = L >> 3;                                                                                   // L is a multiple of 8
-    // row r of this lane as two quads of 4 entries: quads[2 * (r * 32) + h]
-    uint2 *__restrict__ quads = reinterpret_cast<uint2 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + 2 * lane;
+    uint4 *__restrict__ rows = reinterpret_cast<uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;    // row r of this lane: rows[r * 32]
     const int rows_cap = ws.a_cap >> 3;
-    const unsigned long long dummy4 = 0x0001000100010001ull * (unsigned long long)dummy;
     const int fcap = ws.far_cap;
     uint16_t *nbuf = reinterpret_cast<uint16_t *>(smem_raw + (size_t)s_chunk * sizeof(vec4)) +
-                     (size_t)w * NEAR_CAP * 32 + lane;                                   // nbuf[k * 32]
+                     (size_t)w * (NEAR_CAP + FQ) * 32 + lane;                            // nbuf[k * 32]
+    uint16_t *fq = nbuf + NEAR_CAP * 32;                                                 // fq[(k & 15) * 32]
 
     int row_cur = 0, nseg = 0;
     long long slots = 0, slots_far = 0;
     bool bad = false;
     int kf = 0, kn = 0;                  // far / near entries of this lane in the open segment
-    unsigned long long pend = 0;         // the far quad being filled
+    int fw = 0;                          // far entries of this lane already written to its rows (multiple of 8)
 
-    auto put_quad = [&](int q, unsigned long long v) {      // quad q of the open segment's far part
-        const int r = row_cur + (q >> 1);
-        if (r < rows_cap) quads[(size_t)r * 64 + (q & 1)] = make_uint2((unsigned)v, (unsigned)(v >> 32));
+    // this lane's far row fw / 8 of the open segment from the ring; entries from `valid` on are padding
+    auto put_row = [&](int valid) {
+        unsigned v[8];
+#pragma unroll
+        for (int h = 0; h < 8; ++h) v[h] = fw + h < valid ? fq[((fw + h) & (FQ - 1)) * 32] : dummy;
+        const int r = row_cur + (fw >> 3);
+        if (r < rows_cap) rows[(size_t)r * 32] = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
+        fw += 8;
     };
     // closes the open segment: pads both classes to the longest lane, writes the near rows and the descriptor
     auto close_segment = [&](int c) {
@@ -159,10 +166,8 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         if (row_cur + fr + nr > rows_cap || nseg >= NSEG_MAX - 1) {
             bad = true;                                                       // capacity: CLUSTER lists are used
         } else {
-            int q = kf >> 2;                                                  // first far quad not stored yet
-            if (kf & 3) { put_quad(q, pend | (dummy4 << ((kf & 3) * 16))); ++q; }
-            for (; q < 2 * fr; ++q) put_quad(q, dummy4);
-            uint4 *out = reinterpret_cast<uint4 *>(quads) + (size_t)(row_cur + fr) * 32;
+            while (fw < 8 * fr) put_row(kf);                                  // my last (partial) row, then padding rows
+            uint4 *out = rows + (size_t)(row_cur + fr) * 32;
             for (int r = 0; r < nr; ++r, out += 32) {
                 unsigned v[8];
 #pragma unroll
@@ -175,7 +180,7 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             slots += 2 * (ncf + ncn);
             slots_far += 2 * ncf;
         }
-        kf = 0; kn = 0; pend = 0;
+        kf = 0; kn = 0; fw = 0;
     };
 
     for (int c = 0; c < n_chunks; ++c) {
@@ -190,40 +195,27 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             const uint4 cur = nxt;
             if (v + 1 < L8) nxt = ent8[v + 1];           // one address per quarter warp, one load ahead
             const unsigned word[4] = {cur.x, cur.y, cur.z, cur.w};
-            // the 8 entries of the vector are tested together (8 independent chains), then the hits
-            // are appended in list order
-            unsigned loc[8];
-            bool hit[8], far[8];
+            // the 8 entries of the vector are tested together (8 independent chains), then appended
+            // without a branch: a predicated store into the ring / the near buffer and a counter
 #pragma unroll
             for (int h = 0; h < 8; ++h) {
                 const unsigned e = (word[h >> 1] >> ((h & 1) * 16)) & 0xffffu;
-                loc[h] = (e * magic) >> 20;                        // e / n_chunks
-                hit[h] = (int)e < count && e - loc[h] * (unsigned)n_chunks == (unsigned)c;   // padding entries are == count
-                if (h == 7) open = (int)e < count;                 // padding only at the end of a list
-            }
-#pragma unroll
-            for (int h = 0; h < 8; ++h) {
-                const vec4 pj = s_pos[hit[h] ? loc[h] : 0u];
+                const unsigned loc = (e * magic) >> 20;                        // e / n_chunks
+                bool hit = (int)e < count && e - loc * (unsigned)n_chunks == (unsigned)c;   // padding entries are == count
+                if (h == 7) open = (int)e < count;                             // padding only at the end of a list
+                const vec4 pj = s_pos[hit ? loc : 0u];
                 const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
                 const real r2 = Rx * Rx + Ry * Ry + Rz * Rz;
                 const real ww = pi.w * pj.w;
-                hit[h] = hit[h] && r2 <= rc2 && r2 > (real)1e-10;
-                far[h] = ((r2 * r2 * r2) * (ww * ww) >= far_x2 && r2 >= far_r2) || far_r2 < (real)0;    // x^2 = R^6 (w_i w_j)^2
+                hit = hit && r2 <= rc2 && r2 > (real)1e-10;
+                const bool far = ((r2 * r2 * r2) * (ww * ww) >= far_x2 && r2 >= far_r2) || far_r2 < (real)0;    // x^2 = R^6 (w_i w_j)^2
+                const uint16_t off = (uint16_t)(loc * (unsigned)sizeof(vec4));
+                if (hit && far) fq[(kf & (FQ - 1)) * 32] = off;
+                if (hit && !far) nbuf[kn * 32] = off;
+                kf += (hit && far) ? 1 : 0;
+                kn += (hit && !far) ? 1 : 0;
             }
-#pragma unroll
-            for (int h = 0; h < 8; ++h) {
-                if (hit[h]) {
-                    const unsigned off = loc[h] * (unsigned)sizeof(vec4);
-                    if (far[h]) {
-                        pend |= (unsigned long long)off << ((kf & 3) * 16);
-                        if ((kf & 3) == 3) { put_quad(kf >> 2, pend); pend = 0; }
-                        ++kf;
-                    } else {
-                        nbuf[kn * 32] = (uint16_t)off;
-                        ++kn;
-                    }
-                }
-            }
+            if (kf - fw >= 8) put_row(kf);               // at most 15 entries were waiting: one row empties the ring enough
             // a vector adds at most 8 entries to a class: close the segment before pass 2's image or the
             // near buffer could overflow
             if (__any_sync(0xffffffffu, kf > fcap - 8 || kn > NEAR_CAP - 8)) close_segment(c);
@@ -315,7 +307,7 @@ int atom_build(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
     const bool f64 = c->p.precision == TKHP_FP64;
     const int s_chunk = atom_chunk_capacity(f64, ws.chunk_cap);
-    const size_t smem = (size_t)s_chunk * (f64 ? sizeof(double4) : sizeof(float4)) + (size_t)GB * NEAR_CAP * 32 * sizeof(uint16_t);
+    const size_t smem = (size_t)s_chunk * (f64 ? sizeof(double4) : sizeof(float4)) + (size_t)GB * (NEAR_CAP + FQ) * 32 * sizeof(uint16_t);
     const double rc2 = c->p.cutoff * c->p.cutoff;
     // far class off (FP64, beta = 0): far_r2 < 0 puts every pair into the first class of rows, which
     // the kernels then evaluate with the full formula
