@@ -64,6 +64,7 @@ def parse_args():
     ap.add_argument("--tol", type=float, default=1e-6)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-stored-t", action="store_true", help="skip the stored-matrix-elements leg (TKHP_SOLVER_STORED_T)")
     ap.add_argument("--peak-seconds", type=float, default=1.0)
     ap.add_argument("--table", action="store_true",
                     help="instead of the JSON line: the markdown result table of BASELINE.md section 3 "
@@ -480,6 +481,39 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                       "frac": (build_bytes / (phase_ms["build"] * 1e-3) / 1e9 / hbm_gbs) if hbm_gbs and phase_ms["build"] > 0 else None,
                       "note": "190 B/atom (SURVEY 8(d)) + 2 B per list slot written"}
 
+    # ---- the same product with STORED real-space matrix elements (TKHP_SOLVER_STORED_T; SURVEY 8(f) 1b,
+    # PAPER.md L160-162): a second context on the same system, 20 products with the L2 flushed; the
+    # stream (8 B per list slot + the 2 B list entry) is what bounds it, so it goes against the HBM roofline
+    stored_t = None
+    if (rank == 0 and world == 1 and not args.no_stored_t and mode_in_use == pk.TKHP_LIST_ATOM
+            and args.precision != "fp64"):
+        P2 = pk.Polarizer.for_system(sys_, precision=precision, list_mode=want_mode, device=local_rank,
+                                     solver_flags=pk.TKHP_SOLVER_STORED_T)
+        pk.tkhp_nblist_build(P2.ctx, d_pos, d_alpha, d_group, stream)
+        for _ in range(3):
+            pk.tkhp_tmatvec(P2.ctx, d_probe, d_out, stream)        # the first call also computes the elements
+        pk.tkhp_profile_reset(P2.ctx, True)
+        for _ in range(20):
+            flush.fill_(1)
+            pk.tkhp_tmatvec(P2.ctx, d_probe, d_out, stream)
+        torch.cuda.synchronize()
+        pr2 = pk.tkhp_profile_read(P2.ctx)
+        st_ms = pr2["tmatvec_ms"] / max(pr2["n_tmatvec"], 1)
+        pk.tkhp_profile_reset(P2.ctx, True)
+        mu2 = torch.empty((n, 3), dtype=f64, device=dev)
+        it2s, rms2s, _ = pk.tkhp_polar_solve(P2.ctx, d_field, mu2, args.tol, 100, False, stream)
+        torch.cuda.synchronize()
+        st_bytes = 10.0 * n_slots                                  # 8 B of factors + 2 B of list entry per slot
+        stored_t = {"kernel": "k_atom_tmu_stored, one launch per product", "avg_kernel_ms": st_ms,
+                    "launches_timed": pr2["n_tmatvec"], "bytes_per_product": st_bytes, "bound": "hbm",
+                    "achieved_gbs": st_bytes / (st_ms * 1e-3) / 1e9 if st_ms > 0 else None,
+                    "peak_gbs": hbm_gbs,
+                    "frac": st_bytes / (st_ms * 1e-3) / 1e9 / hbm_gbs if hbm_gbs and st_ms > 0 else None,
+                    "vs_recomputing_kernel_ms": mv_kernel_ms,
+                    "solve_ms": P2.timings()["solve"], "solve_iterations": it2s,
+                    "extra_workspace_bytes": P2.workspace_bytes - P.workspace_bytes}
+        P2.close()
+
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -550,7 +584,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "build_roofline": build_roofline,
         "launch_bound": n < 5000,
         "wall_ms_per_step_incl_flush": 1e3 * wall_s / args.steps,
-        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+        "roofline": roofline, "stored_t": stored_t, "cpu_baseline": cpu, "e2e": e2e,
         "gpu_launches": prof_tot["launches"], "clocks": clocks,
     }
     print(json.dumps(line), flush=True)

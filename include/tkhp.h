@@ -97,7 +97,13 @@ typedef struct {
 /* tkhp_params.solver_flags */
 enum {
     TKHP_SOLVER_NO_PERSISTENT = 1, /* never run the solve as one persistent cooperative kernel */
-    TKHP_SOLVER_NO_FUSED_STEP = 2  /* launch-per-matvec path: update and direction as two kernels */
+    TKHP_SOLVER_NO_FUSED_STEP = 2, /* launch-per-matvec path: update and direction as two kernels */
+    TKHP_SOLVER_STORED_T = 4       /* MIXED/FIXED precision, ATOM lists: precompute the real-space matrix elements
+                                      (two radial factors per list slot, 8 bytes) after a list build and stream
+                                      them in every T.mu product instead of re-evaluating the
+                                      radial functions; tkhp_tmatvec and the launch-per-matvec solve use it, the
+                                      persistent solve kernel is not used.  Adds 8 bytes per list slot of capacity
+                                      to the workspace. */
 };
 
 /* Bytes of device workspace tkhp_create() needs for these parameters.  Host, pure. */

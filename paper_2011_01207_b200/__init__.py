@@ -10,7 +10,7 @@ but creating a context without a CUDA device raises, and a missing
 ``libtkhp.so`` raises at import of :mod:`paper_2011_01207_b200.binding`.
 """
 from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_FIXED, TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM,
-                      TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP,
+                      TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP, TKHP_SOLVER_STORED_T,
                       TkhpError, TkhpParams, Polarizer, lib, lib_path,
                       tkhp_workspace_bytes, tkhp_create, tkhp_destroy, tkhp_last_error,
                       tkhp_nblist_build, tkhp_nblist_view, tkhp_nblist_stats, tkhp_nblist_atom_stats,
@@ -20,7 +20,7 @@ from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_FIXED, TKHP_LIST_TILES, TKHP_L
                       EXPORTED_SYMBOLS)
 
 __all__ = [
-    "TKHP_FP64", "TKHP_MIXED", "TKHP_FIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TKHP_LIST_ATOM", "TKHP_SOLVER_NO_PERSISTENT", "TKHP_SOLVER_NO_FUSED_STEP", "TkhpError",
+    "TKHP_FP64", "TKHP_MIXED", "TKHP_FIXED", "TKHP_LIST_TILES", "TKHP_LIST_CLUSTER", "TKHP_LIST_ATOM", "TKHP_SOLVER_NO_PERSISTENT", "TKHP_SOLVER_NO_FUSED_STEP", "TKHP_SOLVER_STORED_T", "TkhpError",
     "TkhpParams", "Polarizer", "lib", "lib_path", "tkhp_workspace_bytes", "tkhp_create",
     "tkhp_destroy", "tkhp_last_error", "tkhp_nblist_build", "tkhp_nblist_view",
     "tkhp_nblist_stats", "tkhp_nblist_atom_stats", "tkhp_perm_field", "tkhp_tmatvec", "tkhp_polar_solve",

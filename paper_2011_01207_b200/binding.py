@@ -11,7 +11,7 @@ TKHP_EINVAL, TKHP_ECUDA, TKHP_ECUTOFF, TKHP_ENOLIST = -1, -2, -3, -4
 TKHP_ENOCONV, TKHP_ECAPACITY, TKHP_ENONFINITE = -5, -6, -7
 TKHP_FP64, TKHP_MIXED, TKHP_FIXED = 0, 1, 2
 TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM = 0, 1, 2
-TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP = 1, 2
+TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP, TKHP_SOLVER_STORED_T = 1, 2, 4
 
 _ERR_NAMES = {-1: "TKHP_EINVAL", -2: "TKHP_ECUDA", -3: "TKHP_ECUTOFF", -4: "TKHP_ENOLIST",
               -5: "TKHP_ENOCONV", -6: "TKHP_ECAPACITY", -7: "TKHP_ENONFINITE"}

@@ -34,7 +34,7 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
     }
     if (p->precision != TKHP_FP64 && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED / FIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }
     if (p->max_tiles_per_block < 0 || p->max_nbrs_per_cluster < 0 || p->max_nbrs_per_atom < 0) { snprintf(err, n, "negative capacity"); return TKHP_EINVAL; }
-    if (p->solver_flags & ~(TKHP_SOLVER_NO_PERSISTENT | TKHP_SOLVER_NO_FUSED_STEP) || p->reserved != 0) { snprintf(err, n, "unknown solver_flags / non-zero reserved field"); return TKHP_EINVAL; }
+    if (p->solver_flags & ~(TKHP_SOLVER_NO_PERSISTENT | TKHP_SOLVER_NO_FUSED_STEP | TKHP_SOLVER_STORED_T) || p->reserved != 0) { snprintf(err, n, "unknown solver_flags / non-zero reserved field"); return TKHP_EINVAL; }
     if (p->max_stage_per_chunk < 0 || (p->max_stage_per_chunk & 31)) { snprintf(err, n, "max_stage_per_chunk must be a non-negative multiple of 32"); return TKHP_EINVAL; }
     return TKHP_OK;
 }
@@ -126,6 +126,11 @@ static size_t carve(Ctx *c, const tkhp_params *p, void *base) {
     o->h_field = w.take<double>(3 * n);
     o->h_mu = w.take<double>(3 * n);
     o->h_energy = w.take<double>(1);
+    {
+        const size_t tb = atom_stored_bytes(p, n_blocks);
+        o->tstore = tb ? w.take<uint4>(tb / sizeof(uint4)) : nullptr;
+        o->stored_t = tb != 0;
+    }
     o->cl_ws_bytes = cluster_workspace_bytes(p, n_blocks);
     o->cl_ws = w.take<char>(o->cl_ws_bytes);
     w.take<char>(256);
@@ -213,7 +218,7 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     c->fixed = params->precision == TKHP_FIXED;
     c->no_persist = (params->solver_flags & TKHP_SOLVER_NO_PERSISTENT) != 0;
     c->no_fused_step = (params->solver_flags & TKHP_SOLVER_NO_FUSED_STEP) != 0;
-    if (cluster_pairs_configure(c) || atom_lists_configure(c) || atom_pairs_configure(c) || atom_solve_configure(c)) {
+    if (cluster_pairs_configure(c) || atom_lists_configure(c) || atom_pairs_configure(c) || atom_solve_configure(c) || atom_stored_configure(c)) {
         snprintf(g_create_err, sizeof(g_create_err), "%s", c->err);
         delete c;
         return TKHP_ECUDA;
@@ -237,6 +242,7 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventCreate(&c->prof_ev[w][i]);
     for (int i = 0; i < 5; ++i) c->last_ms[i] = -1.0;
     c->built = false;
+    c->tstore_valid = false;
     c->header_valid = false;
     c->list_mode_in_use = TKHP_LIST_TILES;
     // the device-resident scalars start from zero (tickets, barrier words: tkhp_polar_energy may be the first call)
@@ -329,6 +335,7 @@ int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polari
         if (rc) return rc;
     }
     c->built = true;
+    c->tstore_valid = false;               // stored matrix elements belong to the previous list
     c->list_mode_in_use = TKHP_LIST_TILES;
     toc(c, 0, s);
     return TKHP_OK;

@@ -507,6 +507,7 @@ int atom_pairs_configure(Ctx *c) {
 
 int atom_tmatvec(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
+    if (c->stored_t && c->p.precision != TKHP_FP64) return atom_stored_tmatvec(c, s);      // TKHP_SOLVER_STORED_T
     return c->p.precision != TKHP_FP64 ? launch_tmu32(c, ws, s) : launch_atom_pairs<double, MODE_TMU>(c, ws, s);
 }
 

@@ -330,7 +330,7 @@ int atom_solve_configure(Ctx *c) {
 
 // Can the persistent kernel run this solve?  (list header on the host: ensure_header has run)
 bool atom_solve_eligible(Ctx *c) {
-    if (!c->coop_ok || c->no_persist || c->p.precision == TKHP_FP64 || c->list_mode_in_use != TKHP_LIST_ATOM) return false;
+    if (!c->coop_ok || c->no_persist || c->stored_t || c->p.precision == TKHP_FP64 || c->list_mode_in_use != TKHP_LIST_ATOM) return false;
     ClusterWs ws = get_ws(c);
     const int s_max = atom_chunk_capacity(false, ws.chunk_cap);
     const int need = c->h_state->max_stage;

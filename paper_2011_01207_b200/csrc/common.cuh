@@ -118,6 +118,9 @@ struct Ctx {
     double far_rmin;
     float far_q[6];         // far fit of erfcx in t = 1/R
     float4 *u32;            // n_pad: operand exchange of the persistent PCG kernel (atom_solve.cu)
+    uint4 *tstore;          // TKHP_SOLVER_STORED_T: (G1, G2/3) of every list slot, [block][row][lane][8] float2 (atom_stored.cu)
+    bool stored_t;          // the stored product is in use (flag set, MIXED/FIXED, ATOM lists requested)
+    bool tstore_valid;      // tstore holds the elements of the current list
     bool fixed;             // TKHP_FIXED: int64 fixed-point accumulators in the FP32 pair kernels and the energy
     bool coop_ok;           // the device supports cooperative launches
     bool no_persist, no_fused_step;   // tkhp_params.solver_flags
@@ -208,6 +211,9 @@ int atom_solve_configure(Ctx *c);
 bool atom_solve_eligible(Ctx *c);
 int atom_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess, double tol, int max_iter, cudaStream_t s);
 int atom_tmatvec(Ctx *c, cudaStream_t s);
+size_t atom_stored_bytes(const tkhp_params *p, int n_blocks);
+int atom_stored_configure(Ctx *c);
+int atom_stored_tmatvec(Ctx *c, cudaStream_t s);
 int atom_field(Ctx *c, cudaStream_t s);
 long long atom_slots(Ctx *c);
 
