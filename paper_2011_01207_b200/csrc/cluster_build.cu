@@ -34,6 +34,8 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
     __shared__ double s_gc[3], s_gh[3];
     __shared__ int s_wsum[GB];
     __shared__ int s_base;
+    __shared__ float4 s_q[2 * GT];        // (e): queue of candidate atoms that passed the group-box test
+    __shared__ int s_qslot[2 * GT];
 
     const int g = blockIdx.x, t = threadIdx.x, lane = t & 31, w = t >> 5;
     const int b0 = ws.group_first[g], nb = ws.group_first[g + 1] - b0;
@@ -161,54 +163,90 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
     __syncthreads();
     const int ncand = s_ncand;
 
-    // (e) every atom of the candidate blocks against the group's clusters
+    // (e) every atom of the candidate blocks against the group's clusters, in two steps.  Step 1 (cheap,
+    // one candidate block per warp): the atom's image in the group frame and a test against the GROUP box;
+    // the survivors (about half of the candidate atoms) are appended, in candidate order, to a queue in
+    // shared memory.  Step 2 (expensive, whenever the queue holds a full CTA of atoms): one queued atom
+    // per thread against the 32 cluster boxes, then against the atoms of the clusters within reach.  All
+    // lanes of step 2 have work, and the staging order is the candidate order, as before.
     const size_t gbase = (size_t)g * ws.s_cap;
-    for (int c0 = 0; c0 < ncand; c0 += GB) {
+    const float ghx = (float)s_gh[0] + 1e-4f, ghy = (float)s_gh[1] + 1e-4f, ghz = (float)s_gh[2] + 1e-4f;
+    const float rcm2_loose = rcm2 * 1.0001f;
+    int q_n = 0;                                       // queued atoms (uniform over the CTA)
+    for (int c0 = 0; c0 < ncand || q_n > 0; c0 += GB) {
+        // ---- step 1
+        if (c0 < ncand) {
+            bool keep = false;
+            float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
+            int slot = -1;
+            if (c0 + w < ncand) {
+                const int J = s_cand[c0 + w];
+                slot = J * BLOCK + lane;
+                const float4 p = xyzw32[slot];
+                if (p.w > 0.f) {
+                    const double4 cj = bcentre[J];
+                    double px = (double)p.x + (cj.x - gcx), py = (double)p.y + (cj.y - gcy), pz = (double)p.z + (cj.z - gcz);
+                    if (f64) {
+                        const double4 q = xyzw64[slot];
+                        px = q.x + (cj.x - gcx); py = q.y + (cj.y - gcy); pz = q.z + (cj.z - gcz);
+                    }
+                    // the image is chosen per ATOM (unique because r_c + group half extent < box/2);
+                    // a per-block shift would be ambiguous when r_c + both extents exceeds box/2
+                    if (box > 0.0) {
+                        px -= box * rint(px / box); py -= box * rint(py / box); pz -= box * rint(pz / box);
+                    }
+                    pj = make_float4((float)px, (float)py, (float)pz, p.w);
+                    const float ex = fmaxf(0.f, fabsf(pj.x) - ghx), ey = fmaxf(0.f, fabsf(pj.y) - ghy), ez = fmaxf(0.f, fabsf(pj.z) - ghz);
+                    keep = ex * ex + ey * ey + ez * ez <= rcm2_loose;
+                }
+            }
+            const unsigned bal = __ballot_sync(0xffffffffu, keep);
+            if (lane == 0) s_wsum[w] = __popc(bal);
+            __syncthreads();
+            int before = 0, total = 0;
+            for (int k = 0; k < GB; ++k) {
+                const int v = s_wsum[k];
+                if (k < w) before += v;
+                total += v;
+            }
+            if (keep) {
+                const int pos = q_n + before + __popc(bal & ((1u << lane) - 1u));
+                s_q[pos] = pj;
+                s_qslot[pos] = slot;
+            }
+            q_n += total;
+            __syncthreads();
+            if (q_n < GT && c0 + GB < ncand) continue;          // wait for a full CTA of queued atoms
+        }
+        // ---- step 2: the first min(GT, q_n) queued atoms
+        const int n_now = min(GT, q_n);
         uint32_t mask = 0;
         float4 pj = make_float4(0.f, 0.f, 0.f, 0.f);
-        double px = 0, py = 0, pz = 0, pw = 0;
         int slot = -1;
-        if (c0 + w < ncand) {
-            const int J = s_cand[c0 + w];
-            slot = J * BLOCK + lane;
-            const float4 p = xyzw32[slot];
-            if (p.w > 0.f) {
-                const double4 cj = bcentre[J];
-                const double dx = cj.x - gcx, dy = cj.y - gcy, dz = cj.z - gcz;
-                if (f64) {
-                    const double4 q = xyzw64[slot];
-                    px = q.x + dx; py = q.y + dy; pz = q.z + dz; pw = q.w;
-                } else {
-                    px = (double)p.x + dx; py = (double)p.y + dy; pz = (double)p.z + dz; pw = p.w;
-                }
-                // the image is chosen per ATOM (unique because r_c + group half extent < box/2);
-                // a per-block shift would be ambiguous when r_c + both extents exceeds box/2
-                if (box > 0.0) {
-                    px -= box * rint(px / box); py -= box * rint(py / box); pz -= box * rint(pz / box);
-                }
-                pj = make_float4((float)px, (float)py, (float)pz, p.w);
-                // first the 32 cluster boxes (uniform loop), then the atoms of the clusters whose box
-                // is within reach (a loop over the set bits: ~1/4 of the clusters)
-                uint32_t near_box = 0;
+        if (t < n_now) {
+            pj = s_q[t];
+            slot = s_qslot[t];
+            // first the 32 cluster boxes (uniform loop), then the atoms of the clusters whose box
+            // is within reach (a loop over the set bits: ~1/4 of the clusters)
+            uint32_t near_box = 0;
 #pragma unroll 8
-                for (int o = 0; o < OCT; ++o) {
-                    const float ex = fmaxf(0.f, fmaxf(s_olo[o][0] - pj.x, pj.x - s_ohi[o][0]));
-                    const float ey = fmaxf(0.f, fmaxf(s_olo[o][1] - pj.y, pj.y - s_ohi[o][1]));
-                    const float ez = fmaxf(0.f, fmaxf(s_olo[o][2] - pj.z, pj.z - s_ohi[o][2]));
-                    if (ex * ex + ey * ey + ez * ez <= rcm2) near_box |= 1u << o;
-                }
-                while (near_box) {
-                    const int o = __ffs(near_box) - 1;
-                    near_box &= near_box - 1;
-                    bool any = false;
+            for (int o = 0; o < OCT; ++o) {
+                const float ex = fmaxf(0.f, fmaxf(s_olo[o][0] - pj.x, pj.x - s_ohi[o][0]));
+                const float ey = fmaxf(0.f, fmaxf(s_olo[o][1] - pj.y, pj.y - s_ohi[o][1]));
+                const float ez = fmaxf(0.f, fmaxf(s_olo[o][2] - pj.z, pj.z - s_ohi[o][2]));
+                if (ex * ex + ey * ey + ez * ez <= rcm2) near_box |= 1u << o;
+            }
+            while (near_box) {
+                const int o = __ffs(near_box) - 1;
+                near_box &= near_box - 1;
+                bool any = false;
 #pragma unroll
-                    for (int a = 0; a < CLUSTER; ++a) {
-                        const float4 q = s_i[o * CLUSTER + a];
-                        const float ddx = q.x - pj.x, ddy = q.y - pj.y, ddz = q.z - pj.z;
-                        any |= (ddx * ddx + ddy * ddy + ddz * ddz <= rcm2) && (q.w > 0.f);
-                    }
-                    if (any) mask |= 1u << o;
+                for (int a = 0; a < CLUSTER; ++a) {
+                    const float4 q = s_i[o * CLUSTER + a];
+                    const float ddx = q.x - pj.x, ddy = q.y - pj.y, ddz = q.z - pj.z;
+                    any |= (ddx * ddx + ddy * ddy + ddz * ddz <= rcm2) && (q.w > 0.f);
                 }
+                if (any) mask |= 1u << o;
             }
         }
         // block-wide exclusive rank of the staged atoms (warp ballots + 8 warp sums)
@@ -227,12 +265,28 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
             if (idx < ws.s_cap - 1) {
                 ws.stage_atom[gbase + idx] = slot;
                 ws.stage_pos32[gbase + idx] = pj;
-                if (f64) ws.stage_pos64[gbase + idx] = make_double4(px, py, pz, pw);
+                if (f64) {
+                    // the FP64 image again (same arithmetic as step 1)
+                    const int J = slot / BLOCK;
+                    const double4 cj = bcentre[J];
+                    const double4 q = xyzw64[slot];
+                    double px = q.x + (cj.x - gcx), py = q.y + (cj.y - gcy), pz = q.z + (cj.z - gcz);
+                    if (box > 0.0) {
+                        px -= box * rint(px / box); py -= box * rint(py / box); pz -= box * rint(pz / box);
+                    }
+                    ws.stage_pos64[gbase + idx] = make_double4(px, py, pz, q.w);
+                }
                 ws.stage_mask[gbase + idx] = mask;
             }
         }
+        // the rest of the queue moves to the front
+        float4 mv = make_float4(0.f, 0.f, 0.f, 0.f);
+        int mvs = -1;
+        if (GT + t < q_n) { mv = s_q[GT + t]; mvs = s_qslot[GT + t]; }
         __syncthreads();
         if (t == 0) s_base = base + total;
+        if (GT + t < q_n) { s_q[t] = mv; s_qslot[t] = mvs; }
+        q_n -= n_now;
         __syncthreads();
     }
     int count = s_base;
