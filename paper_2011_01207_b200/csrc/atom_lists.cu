@@ -260,7 +260,7 @@ k_atom_deal(ClusterWs ws, int n_blocks, int rec_bytes) {
     uint4 *__restrict__ rows = reinterpret_cast<uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;
     const int2 *__restrict__ seg = ws.aseg + (size_t)blk * NSEG_MAX;
     const unsigned dummy = (unsigned)seg[NSEG_MAX - 1].y;            // byte offset of the first dummy record
-    const bool multi = rec_bytes == 16;                              // 16-byte records: one dummy per index class (N_DUMMY)
+    const unsigned rec_shift = rec_bytes == 16 ? 4u : 5u;            // index class of an entry = (offset / record bytes) mod 16
     const unsigned n_loc = dummy / (unsigned)rec_bytes;
     for (int r = 0; r < img_rows; ++r) img[r * 32] = 0xffffu;
     D.clear();
@@ -284,7 +284,7 @@ k_atom_deal(ClusterWs ws, int n_blocks, int rec_bytes) {
                                        e.z & 0xffffu, e.z >> 16, e.w & 0xffffu, e.w >> 16};
 #pragma unroll
                 for (int h = 0; h < 8; ++h)
-                    if (v[h] < dummy) deal(D, img, colcap, l16, v[h], (v[h] >> 4) & 15u);      // (the scan pads with the first dummy)
+                    if (v[h] < dummy) deal(D, img, colcap, l16, v[h], (v[h] >> rec_shift) & 15u);      // (the scan pads with the first dummy)
             }
             level(D, img, l16, (unsigned)len);
             for (int q = 0; q < nrow; ++q) {
@@ -294,7 +294,7 @@ k_atom_deal(ClusterWs ws, int n_blocks, int rec_bytes) {
                     const int e = 8 * q + h;
                     const unsigned x = img[e * 32];
                     // padding: the dummy record of the index class this lane wants at this step
-                    const unsigned pad = multi ? dummy + (((unsigned)(e + lane) - n_loc) & 15u) * 16u : dummy;
+                    const unsigned pad = dummy + ((((unsigned)(e + lane) - n_loc) & 15u) << rec_shift);
                     v[h] = (e >= len || x == 0xffffu) ? pad : x;
                     img[e * 32] = 0xffffu;
                 }

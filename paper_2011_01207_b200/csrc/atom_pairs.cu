@@ -58,6 +58,24 @@ struct Partial {
 //   MODE_TMU   (T1,T2): out_i += -m1 mu_j + m2 (mu_j.R) R            staged: pos+w, mu
 //   MODE_FIELD (F1,F2): field at i from (q,d,Q)_j, same-group pairs contribute zero here (the FP64
 //                       correction pass adds them, pcg.cu)            staged: pos+w, 3 multipole vec4
+// One staged record (4 reals).  FP32: 16 bytes at base + off.  FP64: the record is kept as two 16-byte
+// halves, (x, y) at base + off/2 and (z, w) at base + half + off/2 (half = 16 bytes x records per array),
+// so that a quarter warp's LDS.128 of eight records with different indices mod 8 is one wavefront, as
+// in FP32 (a 32-byte record at a 32-byte stride can never be: only every other bank group is used).
+template <typename real> struct RecLoad;
+template <> struct RecLoad<float> {
+    static __device__ __forceinline__ float4 get(const unsigned char *base, int, unsigned off) {
+        return *reinterpret_cast<const float4 *>(base + off);
+    }
+};
+template <> struct RecLoad<double> {
+    static __device__ __forceinline__ double4 get(const unsigned char *base, int half, unsigned off) {
+        const double2 lo = *reinterpret_cast<const double2 *>(base + (off >> 1));
+        const double2 hi = *reinterpret_cast<const double2 *>(base + half + (off >> 1));
+        return make_double4(lo.x, lo.y, hi.x, hi.y);
+    }
+};
+
 template <typename real, int MODE, int W>
 __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_stride, const unsigned (&off)[W],
                                            const typename Vec4<real>::type &pi, real gi,
@@ -68,11 +86,12 @@ __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_
     vec4 pj[W];
     real Rx[W], Ry[W], Rz[W], r2[W], ww[W], G[W][NK];
 #pragma unroll
-    for (int u = 0; u < W; ++u) pj[u] = *reinterpret_cast<const vec4 *>(s_base + off[u]);
+    const int half = pay_stride >> 1;
+    for (int u = 0; u < W; ++u) pj[u] = RecLoad<real>::get(s_base, half, off[u]);
     if (MODE == MODE_TMU) {
         vec4 mj[W];
 #pragma unroll
-        for (int u = 0; u < W; ++u) mj[u] = *reinterpret_cast<const vec4 *>(s_base + pay_stride + off[u]);
+        for (int u = 0; u < W; ++u) mj[u] = RecLoad<real>::get(s_base + pay_stride, half, off[u]);
 #pragma unroll
         for (int u = 0; u < W; ++u) {
             Rx[u] = pi.x - pj[u].x; Ry[u] = pi.y - pj[u].y; Rz[u] = pi.z - pj[u].z;
@@ -88,9 +107,9 @@ __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_
         bool in[W];
 #pragma unroll
         for (int u = 0; u < W; ++u) {
-            b0v[u] = *reinterpret_cast<const vec4 *>(s_base + pay_stride + off[u]);
-            b1v[u] = *reinterpret_cast<const vec4 *>(s_base + 2 * pay_stride + off[u]);
-            b2v[u] = *reinterpret_cast<const vec4 *>(s_base + 3 * pay_stride + off[u]);
+            b0v[u] = RecLoad<real>::get(s_base + pay_stride, half, off[u]);
+            b1v[u] = RecLoad<real>::get(s_base + 2 * pay_stride, half, off[u]);
+            b2v[u] = RecLoad<real>::get(s_base + 3 * pay_stride, half, off[u]);
         }
 #pragma unroll
         for (int u = 0; u < W; ++u) {
@@ -112,11 +131,12 @@ __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_
 __device__ __forceinline__ void cp_async16(unsigned dst, const void *src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
+// one record into local index l of an array region: FP32 16 bytes at l x 16; FP64 two halves (RecLoad)
 template <int BYTES>
-__device__ __forceinline__ void cp_async_rec(void *dst, const void *src) {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(dst);
-#pragma unroll
-    for (int o = 0; o < BYTES; o += 16) cp_async16(d + o, reinterpret_cast<const unsigned char *>(src) + o);
+__device__ __forceinline__ void cp_async_rec(unsigned char *arr, int half, int l, const void *src) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(arr) + 16u * (unsigned)l;
+    cp_async16(d, src);
+    if (BYTES == 32) cp_async16(d + (unsigned)half, reinterpret_cast<const unsigned char *>(src) + 16);
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -220,8 +240,18 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         far.x = far.y = far.z = (real)(-2.0f * PHANTOM_FAR); far.w = 0;
         zero.x = zero.y = zero.z = zero.w = 0;
         const int dmy = atom_dummy_index(count, n_chunks) + t;
-        s_pos[dmy] = far;
-        for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + dmy] = zero;
+        if (sizeof(real) == 4) {
+            s_pos[dmy] = far;
+            for (int k = 0; k < NPAY; ++k) s_pay[k * pstride + dmy] = zero;
+        } else {                               // two 16-byte halves per record
+            real *lo = reinterpret_cast<real *>(smem_raw + 16 * (size_t)dmy), *hi = reinterpret_cast<real *>(smem_raw + (pay_stride >> 1) + 16 * (size_t)dmy);
+            lo[0] = far.x; lo[1] = far.y; hi[0] = far.z; hi[1] = far.w;
+            for (int k = 0; k < NPAY; ++k) {
+                real *plo = reinterpret_cast<real *>(smem_raw + (size_t)(k + 1) * pay_stride + 16 * (size_t)dmy);
+                real *phi = reinterpret_cast<real *>(smem_raw + (size_t)(k + 1) * pay_stride + (pay_stride >> 1) + 16 * (size_t)dmy);
+                plo[0] = 0; plo[1] = 0; phi[0] = 0; phi[1] = 0;
+            }
+        }
     }
 
     // My rows are part, part + wpb, ... of the block's row stream, whatever segment they fall in; a
@@ -247,13 +277,13 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
 #pragma unroll
             for (int u = 0; u < SU; ++u) {
                 const int idx = i0 + u * GT * n_chunks;
-                if (idx < count) cp_async_rec<sizeof(vec4)>(s_pos + l0 + u * GT, stage_pos + gbase + idx);
+                if (idx < count) cp_async_rec<sizeof(vec4)>(smem_raw, pay_stride >> 1, l0 + u * GT, stage_pos + gbase + idx);
             }
 #pragma unroll
             for (int k = 0; k < NPAY; ++k) {
 #pragma unroll
                 for (int u = 0; u < SU; ++u)
-                    if (a[u] >= 0) cp_async_rec<sizeof(vec4)>(s_pay + k * pstride + l0 + u * GT, data + (size_t)k * n_pad + a[u]);
+                    if (a[u] >= 0) cp_async_rec<sizeof(vec4)>(smem_raw + (size_t)(k + 1) * pay_stride, pay_stride >> 1, l0 + u * GT, data + (size_t)k * n_pad + a[u]);
             }
         }
         cp_async_commit();
