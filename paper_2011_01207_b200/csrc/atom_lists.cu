@@ -99,11 +99,13 @@ __device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16
 // own 16-byte row (8 entries, arrival order; pass 2 permutes them in place) as soon as it has one,
 // NEAR hits into a buffer that waits until the length of the far part of the segment is known.
 constexpr int FQ = 32;                  // entries of a lane's far ring (the last 32 far hits: close_segment moves some of them)
+struct TrueTag { static constexpr bool value = true; };
+struct FalseTag { static constexpr bool value = false; };
 
 template <typename real>
 __global__ void __launch_bounds__(GT)
 k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
-            const typename Vec4<real>::type *__restrict__ stage_pos, real rc2, real far_x2, real far_r2,
+            const typename Vec4<real>::type *__restrict__ stage_pos, real rc2, real far_c, real far_r2,
             int s_chunk, DeviceState *st) {
     using vec4 = typename Vec4<real>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -127,6 +129,7 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     const unsigned magic = ((1u << 20) + (unsigned)n_chunks - 1u) / (unsigned)n_chunks;   // e / n for e < 2^16
     const int slot = blk * BLOCK + lane;
     const vec4 pi = gpos[slot];
+    const real vi = cbrt(pi.w * pi.w);
     const int oct = slot >> 3;
     const int L = active ? ws.oct_len[oct] : 0;
     const uint4 *__restrict__ ent8 = reinterpret_cast<const uint4 *>(ws.entries + (size_t)oct * ws.l_cap);  // 8 entries per load
@@ -193,12 +196,10 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
         kf = 0; kn = 0; fw = 0;
     };
 
-    for (int c = 0; c < n_chunks; ++c) {
-        __syncthreads();
-        for (int l = t, idx = c + t * n_chunks; idx < count; l += GT, idx += GT * n_chunks)
-            s_pos[l] = stage_pos[gbase + idx];
-        __syncthreads();
-        if (!active) continue;
+    // the walk over my cluster's list for chunk c; ONE: the group has a single chunk (the usual case:
+    // entry = local index, no division by the chunk count and no membership test)
+    auto walk_chunk = [&](int c, auto one_tag) {
+        constexpr bool ONE = decltype(one_tag)::value;
         uint4 nxt = L8 > 0 ? ent8[0] : make_uint4(0, 0, 0, 0);
         bool open = true;                                // per lane: its cluster's list has entries left
         for (int v = 0; v < L8 && __any_sync(0xffffffffu, open); ++v) {
@@ -210,15 +211,14 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
 #pragma unroll
             for (int h = 0; h < 8; ++h) {
                 const unsigned e = (word[h >> 1] >> ((h & 1) * 16)) & 0xffffu;
-                const unsigned loc = (e * magic) >> 20;                        // e / n_chunks
-                bool hit = (int)e < count && e - loc * (unsigned)n_chunks == (unsigned)c;   // padding entries are == count
+                const unsigned loc = ONE ? e : (e * magic) >> 20;              // e / n_chunks
+                bool hit = (int)e < count && (ONE || e - loc * (unsigned)n_chunks == (unsigned)c);   // padding entries are == count
                 if (h == 7) open = (int)e < count;                             // padding only at the end of a list
                 const vec4 pj = s_pos[hit ? loc : 0u];
                 const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
                 const real r2 = Rx * Rx + Ry * Ry + Rz * Rz;
-                const real ww = pi.w * pj.w;
                 hit = hit && r2 <= rc2 && r2 > (real)1e-10;
-                const bool far = ((r2 * r2 * r2) * (ww * ww) >= far_x2 && r2 >= far_r2) || far_r2 < (real)0;    // x^2 = R^6 (w_i w_j)^2
+                const bool far = r2 * (vi * pj.w) >= far_c && r2 >= far_r2;     // x^(2/3) = R^2 (w_i w_j)^(2/3); far class off: both thresholds are -1
                 const uint16_t off = (uint16_t)(loc * (unsigned)sizeof(vec4));
                 if (hit && far) fq[(kf & (FQ - 1)) * 32] = off;
                 if (hit && !far) nbuf[kn * 32] = off;
@@ -231,6 +231,19 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             if (__any_sync(0xffffffffu, kf > fcap - 8 || kn > NEAR_CAP - 8)) close_segment(c);
         }
         close_segment(c);
+    };
+    for (int c = 0; c < n_chunks; ++c) {
+        __syncthreads();
+        for (int l = t, idx = c + t * n_chunks; idx < count; l += GT, idx += GT * n_chunks)
+        {
+            vec4 p = stage_pos[gbase + idx];
+            p.w = cbrt(p.w * p.w);                       // the class test wants w^(2/3)
+            s_pos[l] = p;
+        }
+        __syncthreads();
+        if (!active) continue;
+        if (n_chunks == 1) walk_chunk(c, TrueTag());
+        else walk_chunk(c, FalseTag());
     }
     if (active && lane == 0) {
         seg[nseg] = seg[NSEG_MAX - 1] = make_int2(row_cur | (int)(0xffu << 24), (int)dummy);    // terminator (y = the dummy offset); total rows also in the last slot
@@ -321,7 +334,8 @@ int atom_build(Ctx *c, cudaStream_t s) {
     const double rc2 = c->p.cutoff * c->p.cutoff;
     // far class off (FP64, beta = 0): far_r2 < 0 puts every pair into the first class of rows, which
     // the kernels then evaluate with the full formula
-    const double x2 = c->far_on ? c->far_x0 * c->far_x0 : 0.0, r2_far = c->far_on ? c->far_rmin * c->far_rmin : -1.0;
+    // a pair is FAR iff x = R^3 w_i w_j >= x0, tested as R^2 (w_i w_j)^(2/3) >= x0^(2/3), and R >= R_far
+    const double x2 = c->far_on ? cbrt(c->far_x0 * c->far_x0) : -1.0, r2_far = c->far_on ? c->far_rmin * c->far_rmin : -1.0;
     if (f64)
         k_atom_scan<double><<<ws.n_groups, GT, smem, s>>>(ws, ws.gpos64, ws.stage_pos64, rc2, x2, r2_far, s_chunk, c->st);
     else
