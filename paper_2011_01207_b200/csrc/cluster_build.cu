@@ -27,7 +27,7 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
                 const double4 *__restrict__ bcentre, const double4 *__restrict__ bhalf,
                 const double4 *__restrict__ scentre, const double4 *__restrict__ shalf, int n_blocks,
                 int n_super, double box, double cutoff, DeviceState *st) {
-    __shared__ float4 s_i[GT];
+    __shared__ float4 s_i[GT + OCT];      // atom a of cluster o at o * 9 + a: lanes that read different clusters hit different bank groups
     __shared__ float s_olo[OCT][3], s_ohi[OCT][3];
     __shared__ int s_cand[CB_CAP];
     __shared__ int s_ncand;
@@ -88,7 +88,7 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
             }
             ws.gpos32[slot] = v;
         }
-        s_i[t] = v;
+        s_i[(t >> 3) * 9 + (t & 7)] = v;
     }
     __syncthreads();
 
@@ -96,7 +96,7 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
     if (t < OCT) {
         float lo[3] = {3e38f, 3e38f, 3e38f}, hi[3] = {-3e38f, -3e38f, -3e38f};
         for (int a = 0; a < CLUSTER; ++a) {
-            const float4 q = s_i[t * CLUSTER + a];
+            const float4 q = s_i[t * 9 + a];
             if (q.w > 0.f) {
                 lo[0] = fminf(lo[0], q.x); hi[0] = fmaxf(hi[0], q.x);
                 lo[1] = fminf(lo[1], q.y); hi[1] = fmaxf(hi[1], q.y);
@@ -242,7 +242,7 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
                 bool any = false;
 #pragma unroll
                 for (int a = 0; a < CLUSTER; ++a) {
-                    const float4 q = s_i[o * CLUSTER + a];
+                    const float4 q = s_i[o * 9 + a];
                     const float ddx = q.x - pj.x, ddy = q.y - pj.y, ddz = q.z - pj.z;
                     any |= (ddx * ddx + ddy * ddy + ddz * ddz <= rcm2) && (q.w > 0.f);
                 }
