@@ -87,6 +87,10 @@ static size_t carve(Ctx *c, const tkhp_params *p, void *base) {
     o->cell_start = w.take<uint32_t>(n_cells + 2);
     o->scan_tmp = w.take<uint32_t>((bins + 2) / 2048 + 2);
     o->tmp_idx = w.take<int32_t>(n);
+    o->key2 = w.take<uint32_t>(n);
+    o->count2 = w.take<uint32_t>(n + 2);
+    o->scan_tmp2 = w.take<uint32_t>((n + 2) / 2048 + 2);
+    o->tmp_idx2 = w.take<int32_t>(n);
     o->perm = w.take<int32_t>(n_pad);
     o->pos_o = w.take<double>(3 * n);
     o->group_o = w.take<int32_t>(n);
@@ -238,6 +242,11 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     for (int i = 0; i < 10; ++i) cudaEventCreate(&c->ev[i]);
     cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
     for (int i = 0; i < 2; ++i) cudaEventCreateWithFlags(&c->copy_ev[i], cudaEventDisableTiming);
+    for (int i = 0; i < 2; ++i) {
+        cudaStreamCreateWithFlags(&c->side[i], cudaStreamNonBlocking);
+        cudaEventCreateWithFlags(&c->fork_ev[i], cudaEventDisableTiming);
+        cudaEventCreateWithFlags(&c->join_ev[i], cudaEventDisableTiming);
+    }
     for (int w = 0; w < 3; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventCreate(&c->prof_ev[w][i]);
     for (int i = 0; i < 5; ++i) c->last_ms[i] = -1.0;
@@ -259,6 +268,7 @@ int tkhp_destroy(tkhp_ctx *ctx) {
     cudaDeviceSynchronize();
     for (int i = 0; i < 10; ++i) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 2; ++i) cudaEventDestroy(c->copy_ev[i]);
+    for (int i = 0; i < 2; ++i) { cudaStreamDestroy(c->side[i]); cudaEventDestroy(c->fork_ev[i]); cudaEventDestroy(c->join_ev[i]); }
     cudaStreamDestroy(c->copy_stream);
     for (int w = 0; w < 3; ++w)
         for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventDestroy(c->prof_ev[w][i]);
@@ -279,16 +289,12 @@ const char *tkhp_last_error(const tkhp_ctx *ctx) {
 static int enqueue_build(Ctx *c, const double *d_pos, const double *d_polarizability, const int32_t *d_group_id,
                          cudaStream_t s) {
     int rc = nblist_build(c, d_pos, d_polarizability, d_group_id, s);
-    if (rc) return rc;
-    if (c->p.list_mode != TKHP_LIST_TILES) {
+    if (rc == TKHP_OK && c->p.list_mode != TKHP_LIST_TILES) {
         rc = cluster_build(c, s);
-        if (rc) return rc;
-        if (c->p.list_mode == TKHP_LIST_ATOM) {
-            rc = atom_build(c, s);
-            if (rc) return rc;
-        }
+        if (rc == TKHP_OK && c->p.list_mode == TKHP_LIST_ATOM) rc = atom_build(c, s);
     }
-    return TKHP_OK;
+    const int rj = nblist_join(c, s);          // always: a forked branch must rejoin (stream capture)
+    return rc ? rc : rj;
 }
 
 int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polarizability,

@@ -81,6 +81,9 @@ struct Ctx {
     uint32_t *cell_start;   // n_cells_alloc + 1
     uint32_t *scan_tmp;     // block sums for the scan
     int32_t *tmp_idx;       // N
+    // scratch of the polarization-group sort, which runs beside the spatial sort (side stream / graph branch)
+    uint32_t *key2, *count2, *scan_tmp2;   // N, N + 2, block sums
+    int32_t *tmp_idx2;      // N
     int32_t *perm;          // n_pad, -1 = phantom
     // copies of the caller's build inputs in ORIGINAL order (the list is valid for these positions)
     double *pos_o;          // 3 N
@@ -131,6 +134,11 @@ struct Ctx {
     // host-entry staging (tkhp_polarize_host)
     double *h_pos, *h_alpha, *h_charge, *h_dipole, *h_quad, *h_field, *h_mu, *h_energy;
     cudaStream_t copy_stream;   // tkhp_polarize_host: the multipole H2D copies run beside the list build
+    // list build: two branches beside the critical path (sort -> gather -> finer lists): [0] copies of the
+    // inputs and the polarization-group sort, [1] the prescribed block-pair search (the finer lists do not
+    // read it).  Forked and joined with events, also inside the captured graph.
+    cudaStream_t side[2];
+    cudaEvent_t fork_ev[2], join_ev[2];
     cudaEvent_t copy_ev[2];
     int32_t *h_group;
     // CLUSTER mode lists (see cluster.cu)
@@ -194,6 +202,7 @@ inline int div_up(long long a, long long b) { return (int)((a + b - 1) / b); }
 // ---- host-side launchers implemented in the other translation units ----
 int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32_t *d_group,
                  cudaStream_t s);
+int nblist_join(Ctx *c, cudaStream_t s);            // the caller's stream waits for the two side branches of nblist_build
 int nblist_count_pairs(Ctx *c, cudaStream_t s);
 int tiles_tmatvec(Ctx *c, cudaStream_t s);          // acc = T_real * (mu32|mu64), sorted space
 int tiles_field(Ctx *c, cudaStream_t s);            // acc = unmasked inter-group field

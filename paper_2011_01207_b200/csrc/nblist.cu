@@ -482,8 +482,6 @@ int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32
     const tkhp_params &p = c->p;
     const int nb256 = div_up(n, 256);
     c->header_valid = false;
-    TKHP_CUDA(c, cudaMemcpyAsync(c->pos_o, d_pos, sizeof(double) * 3 * (size_t)n, cudaMemcpyDeviceToDevice, s));
-    TKHP_CUDA(c, cudaMemcpyAsync(c->group_o, d_group, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToDevice, s));
 
     // grid parameters: periodic -> host; open -> device reduction
     if (p.box > 0.0) {
@@ -498,17 +496,24 @@ int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32
         k_grid_from_extent<<<1, 1, 0, s>>>(c->st, b_max);
         c->n_launches += 3;
     }
+    // ---- branch 0 (beside the spatial sort): copies of the inputs in the caller's order, and the members
+    // of every polarization group sorted by (group, index) for the mask correction (A6)
+    {
+        cudaStream_t b = c->side[0];
+        TKHP_CUDA(c, cudaEventRecord(c->fork_ev[0], s));
+        TKHP_CUDA(c, cudaStreamWaitEvent(b, c->fork_ev[0], 0));
+        TKHP_CUDA(c, cudaMemcpyAsync(c->pos_o, d_pos, sizeof(double) * 3 * (size_t)n, cudaMemcpyDeviceToDevice, b));
+        TKHP_CUDA(c, cudaMemcpyAsync(c->group_o, d_group, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToDevice, b));
+        TKHP_CUDA(c, cudaMemsetAsync(c->count2, 0, sizeof(uint32_t) * ((size_t)n + 1), b));
+        k_group_keys<<<nb256, 256, 0, b>>>(d_group, n, c->key2, c->count2);
+        counting_sort(c, c->key2, n, (uint32_t)n, c->count2, c->grp_start, c->scan_tmp2, c->tmp_idx2, c->grp_members, b);
+        TKHP_CUDA(c, cudaEventRecord(c->join_ev[0], b));
+    }
     TKHP_CUDA(c, cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * ((size_t)c->n_cells_alloc + 1), s));
     k_cell_keys<<<nb256, 256, 0, s>>>(d_pos, d_alpha, d_group, n, p.box, c->st, c->key, c->cell_count);
     counting_sort(c, c->key, n, (uint32_t)c->n_cells_alloc, c->cell_count, c->cell_start, c->scan_tmp,
                   c->tmp_idx, c->perm, s);
     if (c->n_pad > n) { k_fill_i32<<<1, 32, 0, s>>>(c->perm + n, c->n_pad - n, -1); c->n_launches += 1; }
-
-    // polarization groups: members sorted by (group, index)
-    TKHP_CUDA(c, cudaMemsetAsync(c->cell_count, 0, sizeof(uint32_t) * ((size_t)n + 1), s));
-    k_group_keys<<<nb256, 256, 0, s>>>(d_group, n, c->key, c->cell_count);
-    counting_sort(c, c->key, n, (uint32_t)n, c->cell_count, c->grp_start, c->scan_tmp, c->tmp_idx,
-                  c->grp_members, s);
 
     // gather + boxes
     const int warps_per_cta = 8;
@@ -518,7 +523,12 @@ int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32
     k_super_boxes<<<div_up(c->n_super, warps_per_cta), warps_per_cta * 32, 0, s>>>(
         c->bcentre, c->bhalf, c->n_blocks, c->n_super, c->scentre, c->shalf);
 
-    // block pairs: count, scan, fill
+    // ---- branch 1: the prescribed block-pair list (count, scan, fill).  The finer lists are built from the
+    // boxes, not from this list, so it runs beside them; the main stream does not touch scan_tmp any more.
+    cudaStream_t s_main = s;
+    s = c->side[1];
+    TKHP_CUDA(c, cudaEventRecord(c->fork_ev[1], s_main));
+    TKHP_CUDA(c, cudaStreamWaitEvent(s, c->fork_ev[1], 0));
     const double reach = p.cutoff + p.skin;
     const double reach2 = reach * reach;
     const double reach_super = reach * (1.0 + 1e-12) + 1e-9;
@@ -533,8 +543,15 @@ int nblist_build(Ctx *c, const double *d_pos, const double *d_alpha, const int32
         c->bcentre, c->bhalf, c->scentre, c->shalf, c->n_blocks, c->n_super, p.box, reach2, reach2_super,
         c->row_count, c->row_start, c->pairs, c->cap_tiles, c->st);
     k_list_finish<<<1, 1, 0, s>>>(c->st, c->row_start, c->n_blocks, c->cap_tiles, p.box, p.cutoff);
+    TKHP_CUDA(c, cudaEventRecord(c->join_ev[1], s));
     c->n_launches += 7;   // cell keys, group keys, gather, super boxes, 2 x pair search, finish
     TKHP_CUDA(c, cudaGetLastError());
+    return TKHP_OK;
+}
+
+int nblist_join(Ctx *c, cudaStream_t s) {
+    TKHP_CUDA(c, cudaStreamWaitEvent(s, c->join_ev[0], 0));
+    TKHP_CUDA(c, cudaStreamWaitEvent(s, c->join_ev[1], 0));
     return TKHP_OK;
 }
 
