@@ -255,7 +255,7 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     c->header_valid = false;
     c->list_mode_in_use = TKHP_LIST_TILES;
     // the device-resident scalars start from zero (tickets, barrier words: tkhp_polar_energy may be the first call)
-    if (cudaMemset(c->st, 0, sizeof(DeviceState)) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) { delete c; return TKHP_ECUDA; }
+    if (cudaMemset(c->st, 0, sizeof(DeviceState)) != cudaSuccess || cluster_init(c) != TKHP_OK || cudaDeviceSynchronize() != cudaSuccess) { delete c; return TKHP_ECUDA; }
     if (prev_device >= 0 && prev_device != params->device) cudaSetDevice(prev_device);      // leave the caller's current device as it was
     *out = reinterpret_cast<tkhp_ctx *>(c);
     return TKHP_OK;

@@ -346,10 +346,18 @@ size_t cluster_workspace_bytes(const tkhp_params *p, int n_blocks) {
 
 int cluster_build(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
-    k_group_first<<<div_up(ws.n_groups + 1, 256), 256, 0, s>>>(ws.group_first, ws.n_groups, c->n_blocks);
     k_cluster_build<<<ws.n_groups, GT, 0, s>>>(ws, c->xyzw32, c->xyzw64, c->bcentre, c->bhalf, c->scentre,
                                                c->shalf, c->n_blocks, c->n_super, c->p.box, c->p.cutoff, c->st);
-    c->n_launches += 2;
+    c->n_launches += 1;
+    TKHP_CUDA(c, cudaGetLastError());
+    return TKHP_OK;
+}
+
+// first block of every group: fixed for the life of the context (tkhp_create, which synchronises)
+int cluster_init(Ctx *c) {
+    if (c->p.list_mode == TKHP_LIST_TILES) return TKHP_OK;
+    ClusterWs ws = get_ws(c);
+    k_group_first<<<div_up(ws.n_groups + 1, 256), 256>>>(ws.group_first, ws.n_groups, c->n_blocks);
     TKHP_CUDA(c, cudaGetLastError());
     return TKHP_OK;
 }

@@ -208,6 +208,7 @@ int tiles_tmatvec(Ctx *c, cudaStream_t s);          // acc = T_real * (mu32|mu64
 int tiles_field(Ctx *c, cudaStream_t s);            // acc = unmasked inter-group field
 size_t cluster_workspace_bytes(const tkhp_params *p, int n_blocks);
 int cluster_build(Ctx *c, cudaStream_t s);
+int cluster_init(Ctx *c);
 int cluster_tmatvec(Ctx *c, cudaStream_t s);
 int cluster_field(Ctx *c, cudaStream_t s);
 long long cluster_slots(Ctx *c);
