@@ -239,12 +239,22 @@ k_cluster_build(ClusterWs ws, const float4 *__restrict__ xyzw32, const double4 *
             while (near_box) {
                 const int o = __ffs(near_box) - 1;
                 near_box &= near_box - 1;
+                // (phantom atoms sit at PHANTOM_FAR: no test of w needed); two halves: most clusters whose
+                // box is within reach have an atom within reach among the first four
                 bool any = false;
 #pragma unroll
-                for (int a = 0; a < CLUSTER; ++a) {
+                for (int a = 0; a < CLUSTER / 2; ++a) {
                     const float4 q = s_i[o * 9 + a];
                     const float ddx = q.x - pj.x, ddy = q.y - pj.y, ddz = q.z - pj.z;
-                    any |= (ddx * ddx + ddy * ddy + ddz * ddz <= rcm2) && (q.w > 0.f);
+                    any |= ddx * ddx + ddy * ddy + ddz * ddz <= rcm2;
+                }
+                if (!any) {
+#pragma unroll
+                    for (int a = CLUSTER / 2; a < CLUSTER; ++a) {
+                        const float4 q = s_i[o * 9 + a];
+                        const float ddx = q.x - pj.x, ddy = q.y - pj.y, ddz = q.z - pj.z;
+                        any |= ddx * ddx + ddy * ddy + ddz * ddz <= rcm2;
+                    }
                 }
                 if (any) mask |= 1u << o;
             }
