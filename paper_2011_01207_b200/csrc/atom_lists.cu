@@ -99,8 +99,6 @@ __device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16
 // own 16-byte row (8 entries, arrival order; pass 2 permutes them in place) as soon as it has one,
 // NEAR hits into a buffer that waits until the length of the far part of the segment is known.
 constexpr int FQ = 32;                  // entries of a lane's far ring (the last 32 far hits: close_segment moves some of them)
-struct TrueTag { static constexpr bool value = true; };
-struct FalseTag { static constexpr bool value = false; };
 
 template <typename real>
 __global__ void __launch_bounds__(GT)

@@ -76,7 +76,7 @@ template <> struct RecLoad<double> {
     }
 };
 
-template <typename real, int MODE, int W>
+template <typename real, int MODE, int W, bool THOLE>
 __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_stride, const unsigned (&off)[W],
                                            const typename Vec4<real>::type &pi, real gi,
                                            const PairConsts<real> &kc, Partial<real> &A) {
@@ -98,7 +98,7 @@ __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_
             r2[u] = Rx[u] * Rx[u] + Ry[u] * Ry[u] + Rz[u] * Rz[u];
             ww[u] = pi.w * pj[u].w;
         }
-        radial_w<NK, W>(r2, ww, kc, G);
+        radial_w<NK, W, THOLE>(r2, ww, kc, G);
 #pragma unroll
         for (int u = 0; u < W; ++u)
             tmu_apply<real>(G[u][0], G[u][1], Rx[u], Ry[u], Rz[u], mj[u].x, mj[u].y, mj[u].z, ax, ay, az);
@@ -118,7 +118,7 @@ __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_
             ww[u] = pi.w * pj[u].w;
             in[u] = b2v[u].z != gi;
         }
-        radial_w<NK, W>(r2, ww, kc, G);
+        radial_w<NK, W, THOLE>(r2, ww, kc, G);
 #pragma unroll
         for (int u = 0; u < W; ++u) {
             if (!in[u]) { G[u][0] = 0; G[u][1] = 0; G[u][2] = 0; }
@@ -298,23 +298,29 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
 #pragma unroll
             for (int cls = 0; cls < 2; ++cls) {
                 const int rend = r0[cls] + ((nc[cls] + 3) >> 2);
-                for (; tg < rend; tg += wpb) {
-                    const uint4 e = e_next;
-                    e_next = ldg_row(rows + (size_t)min(tg + wpb, rows_last) * 32);
-                    const int n_here = min(4, nc[cls] - 4 * (tg - r0[cls]));
-                    const unsigned wd[4] = {e.x, e.y, e.z, e.w};
+                // the rows of one class; THOLE = false for FAR rows (the Thole term has died out)
+                auto rows_of_class = [&](auto thole_tag) {
+                    constexpr bool THOLE = decltype(thole_tag)::value;
+                    for (; tg < rend; tg += wpb) {
+                        const uint4 e = e_next;
+                        e_next = ldg_row(rows + (size_t)min(tg + wpb, rows_last) * 32);
+                        const int n_here = min(4, nc[cls] - 4 * (tg - r0[cls]));
+                        const unsigned wd[4] = {e.x, e.y, e.z, e.w};
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        if (k < n_here) {
-                            const unsigned o2[2] = {wd[k] & 0xffffu, wd[k] >> 16};
-                            eval_pairs<real, MODE, 2>(s_base, pay_stride, o2, pi, gi, kc, A);
+                        for (int k = 0; k < 4; ++k) {
+                            if (k < n_here) {
+                                const unsigned o2[2] = {wd[k] & 0xffffu, wd[k] >> 16};
+                                eval_pairs<real, MODE, 2, THOLE>(s_base, pay_stride, o2, pi, gi, kc, A);
+                            }
+                        }
+                        if (++since_flush == 4) {          // every 32 entries: FP32 partial -> 64-bit container
+                            A.flush(dx, dy, dz, fixed);
+                            since_flush = 0;
                         }
                     }
-                    if (++since_flush == 4) {          // every 32 entries: FP32 partial -> 64-bit container
-                        A.flush(dx, dy, dz, fixed);
-                        since_flush = 0;
-                    }
-                }
+                };
+                if (cls == 0 && kc.far_rows) rows_of_class(FalseTag());
+                else rows_of_class(TrueTag());
             }
             sd = seg[++d];
         }
@@ -435,6 +441,7 @@ void atom_far_setup(Ctx *c) {
     c->far_x0 = 0.0;
     c->far_rmin = 0.0;
     for (int k = 0; k < 6; ++k) c->far_q[k] = 0.f;
+    // (FP64 with a Thole-free first class, x >= 45, was measured: T.mu 0.191 -> 0.213 ms on config 2; not used)
     if (c->p.precision == TKHP_FP64 || !(beta > 0.0) || z_max < 1.25 * z_min) return;    // no far class: full formula everywhere
     c->far_on = true;
     constexpr int D = 5;
@@ -477,6 +484,7 @@ static int launch_atom_pairs(Ctx *c, const ClusterWs &ws, cudaStream_t s) {
     k.inv_box = (real)0;
     k.pb = k.nb2l = k.c1b = k.k3 = (real)0;
     k.fixed = c->fixed ? 1 : 0;
+    k.far_rows = c->far_on ? 1 : 0;
     PcgFuse fuse;
     fuse.on = MODE == MODE_TMU && c->fuse_q;
     fuse.self = 4.0 * c->p.ewald_beta * c->p.ewald_beta * c->p.ewald_beta / (3.0 * SQRT_PI);

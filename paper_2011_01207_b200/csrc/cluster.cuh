@@ -29,6 +29,10 @@
 
 namespace tkhp {
 
+// compile-time flags handed to generic lambdas (one loop body, two instantiations, one uniform branch outside)
+struct TrueTag { static constexpr bool value = true; };
+struct FalseTag { static constexpr bool value = false; };
+
 constexpr int GB = 8;                 // max blocks per group (= warps per CTA)
 constexpr int GT = GB * 32;           // threads per CTA
 constexpr int OCT = GB * 4;           // clusters per group

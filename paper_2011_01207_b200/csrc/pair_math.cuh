@@ -39,6 +39,7 @@ struct PairConsts {
     real c1b;       // (2/sqrt pi) beta:        c z = c1b R
     real k3;        // (4/(3 sqrt pi)) beta^3:  (2c/3) z^3 = k3 R^3
     int fixed;      // TKHP_FIXED (FP32 kernels only): int64 fixed-point accumulators (common.cuh acc_add)
+    int far_rows;   // ATOM lists: the first class of rows holds pairs whose Thole damping has died out (THOLE = false)
 };
 
 template <typename real> struct Vec4;
@@ -76,7 +77,9 @@ __device__ __forceinline__ float erfcx_f32(float z) {
 // dependency chains (the Horner chain alone is 8 dependent FFMAs); W = 2 in the cluster kernels.
 // Scaled forms: R^3 G1 = ez g1 - et;  R^5 G2 / 3 = ez (g1 + (2c/3) z^3) - (1+x) et;
 // R^7 G3 / 15 = ez (g1 + (2c/3) z^3 + (4c/15) z^5) - (1 + x + 0.6 x^2) et.
-template <int NK, int W>
+// THOLE = false (FAR rows of the ATOM lists): x = R^3 w_i w_j is so large that e^-x is below the
+// resolution of the sums; the Thole exponential and its polynomial are skipped (lambda = 1).
+template <int NK, int W, bool THOLE = true>
 __device__ __forceinline__ void radial_f32_w(const float (&r2)[W], const float (&ww)[W],
                                              const PairConsts<float> &k, float (&G)[W][NK]) {
     constexpr float c[TKHP_ERFCX_DEG + 1] = TKHP_ERFCX_COEFFS;
@@ -93,9 +96,9 @@ __device__ __forceinline__ void radial_f32_w(const float (&r2)[W], const float (
 #pragma unroll
     for (int i = 0; i < W; ++i) { z2[i] = z[i] * z[i]; t[i] = r2[i] * r[i]; }
 #pragma unroll
-    for (int i = 0; i < W; ++i) { ez[i] = fast_ex2(z2[i] * NLOG2E); x[i] = t[i] * ww[i]; }
+    for (int i = 0; i < W; ++i) { ez[i] = fast_ex2(z2[i] * NLOG2E); x[i] = THOLE ? t[i] * ww[i] : 0.f; }
 #pragma unroll
-    for (int i = 0; i < W; ++i) { et[i] = fast_ex2(x[i] * NLOG2E); p[i] = c[TKHP_ERFCX_DEG]; }
+    for (int i = 0; i < W; ++i) { et[i] = THOLE ? fast_ex2(x[i] * NLOG2E) : 0.f; p[i] = c[TKHP_ERFCX_DEG]; }
 #pragma unroll
     for (int d = TKHP_ERFCX_DEG - 1; d >= 0; --d) {
 #pragma unroll
@@ -159,7 +162,7 @@ __device__ __forceinline__ double exp_neg(double y) {
     return __hiloint2double(hi, __double2loint(p));
 }
 
-template <int NK>
+template <int NK, bool THOLE = true>
 __device__ __forceinline__ void radial_f64(double r2, double ww, const PairConsts<double> &k, double *G) {
     constexpr double c[TKHP_ERFCX64_DEG + 1] = TKHP_ERFCX64_COEFFS;
     const double rinv = rsqrt(r2);
@@ -175,8 +178,8 @@ __device__ __forceinline__ void radial_f64(double r2, double ww, const PairConst
     for (int d = TKHP_ERFCX64_DEG - 1; d >= 0; --d) p = fma(p, u, c[d]);
     const double cz = k.c1 * z;
     const double B1 = ez * (p + cz);                       // erfc(z) + c z e^{-z^2}
-    const double x = (r2 * r) * ww;
-    const double et = exp_neg(-x);
+    const double x = THOLE ? (r2 * r) * ww : 0.0;
+    const double et = THOLE ? exp_neg(-x) : 0.0;
     const double rinv3 = rinv2 * rinv;
     G[0] = (B1 - et) * rinv3;
     if (NK >= 2) {
@@ -194,16 +197,16 @@ template <int NK>
 __device__ __forceinline__ void radial(float r2, float ww, const PairConsts<float> &k, float *G) {
     radial_f32<NK>(r2, ww, k, G);
 }
-template <int NK, int W>
+template <int NK, int W, bool THOLE = true>
 __device__ __forceinline__ void radial_w(const float (&r2)[W], const float (&ww)[W], const PairConsts<float> &k,
                                          float (&G)[W][NK]) {
-    radial_f32_w<NK, W>(r2, ww, k, G);
+    radial_f32_w<NK, W, THOLE>(r2, ww, k, G);
 }
-template <int NK, int W>
+template <int NK, int W, bool THOLE = true>
 __device__ __forceinline__ void radial_w(const double (&r2)[W], const double (&ww)[W], const PairConsts<double> &k,
                                          double (&G)[W][NK]) {
 #pragma unroll
-    for (int i = 0; i < W; ++i) radial_f64<NK>(r2[i], ww[i], k, G[i]);
+    for (int i = 0; i < W; ++i) radial_f64<NK, THOLE>(r2[i], ww[i], k, G[i]);
 }
 template <int NK>
 __device__ __forceinline__ void radial(double r2, double ww, const PairConsts<double> &k, double *G) {
