@@ -417,7 +417,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         # the whole solve is ONE launch of k_pcg_persist: its T.mu products are the algorithmic work
         kern_ms = prof_tot["solve_ms"] / prof_tot["n_solve"]
         mv_per_launch = prof_tot["solve_matvecs"] / prof_tot["n_solve"]
-        kernel_name = "k_pcg_persist (whole PCG solve: %.1f T.mu products + vector updates, one cooperative launch)" % mv_per_launch
+        kernel_name = "%s (whole PCG solve: %.1f T.mu products + vector updates, one cooperative launch)" % (
+            "k_pcg_persist" if mode_in_use == pk.TKHP_LIST_ATOM else "k_pcg_tiles", mv_per_launch)
         share = prof_tot["solve_ms"] / total_ms if world == 1 else None
         n_timed = prof_tot["n_solve"]
     else:

@@ -48,44 +48,6 @@ struct SolveArgs {
     int max_iter, n_atoms, n_pad, s_chunk, rot_div;
 };
 
-__device__ __forceinline__ unsigned ld_acquire(const unsigned *p) {
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-// All threads of all CTAs.  `gen` counts the barriers this CTA has passed.  One atomic per CTA on a
-// counter that only grows during a solve; everybody spins on the counter itself (one L2 round trip
-// less on the critical path than a separate release word written by the last arriver).
-__device__ __forceinline__ void grid_barrier(DeviceState *st, unsigned &gen) {
-    __syncthreads();
-    ++gen;
-    if (threadIdx.x == 0) {
-        __threadfence();
-        const unsigned target = gen * gridDim.x;
-        if (atomicAdd(&st->bar_count, 1u) + 1u != target) {
-            // bounded spin (a few seconds): a CTA that never arrives must not hang the device
-            for (unsigned n = 0; ld_acquire(&st->bar_count) < target; ++n)
-                if (n > (1u << 22)) { st->err_barrier = 1; break; }
-        }
-        __threadfence();
-    }
-    __syncthreads();
-}
-
-// identical in every CTA: sum of the per-CTA partials in a fixed order
-__device__ __forceinline__ void grid_totals(const double *part, double &a, double &b) {
-    __shared__ double s_tot[2];
-    double x = 0, y = 0;
-    for (int i = threadIdx.x; i < (int)gridDim.x; i += RED_THREADS) {
-        x += __ldcg(part + 2 * i);
-        y += __ldcg(part + 2 * i + 1);
-    }
-    block_sum2(x, y);
-    if (threadIdx.x == 0) { s_tot[0] = x; s_tot[1] = y; }
-    __syncthreads();
-    a = s_tot[0]; b = s_tot[1];
-}
-
 __host__ __device__ inline size_t solve_smem(int s_chunk, bool split) {
     size_t b = ((size_t)TMU_REC * (s_chunk + N_DUMMY) + 15) & ~(size_t)15;   // A, B, W
     b += (size_t)4 * s_chunk;                                         // staging indices

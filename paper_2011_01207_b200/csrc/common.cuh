@@ -219,6 +219,8 @@ int atom_pairs_configure(Ctx *c);
 int cluster_pairs_configure(Ctx *c);
 int atom_solve_configure(Ctx *c);
 bool atom_solve_eligible(Ctx *c);
+bool tiles_solve_eligible(Ctx *c);
+int tiles_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess, double tol, int max_iter, cudaStream_t s);
 int atom_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess, double tol, int max_iter, cudaStream_t s);
 int atom_tmatvec(Ctx *c, cudaStream_t s);
 size_t atom_stored_bytes(const tkhp_params *p, int n_blocks);

@@ -468,10 +468,12 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
     // ---- the whole solve as one persistent cooperative kernel (atom_solve.cu) when it can run: it
     // reads the field and the guess and writes mu in the caller's order, the scalars come back
     // through host-mapped memory
-    if (atom_solve_eligible(c)) {
+    const bool persist_atom = atom_solve_eligible(c);
+    if (persist_atom || tiles_solve_eligible(c)) {
         const bool rec = c->prof && c->prof_n[2] < PROF_MAX;
         if (rec) cudaEventRecord(c->prof_ev[2][2 * c->prof_n[2]], s);
-        rc = atom_solve_launch(c, d_field, d_mu, use_guess, tol, max_iter, s);
+        rc = persist_atom ? atom_solve_launch(c, d_field, d_mu, use_guess, tol, max_iter, s)
+                          : tiles_solve_launch(c, d_field, d_mu, use_guess, tol, max_iter, s);
         if (rec) { cudaEventRecord(c->prof_ev[2][2 * c->prof_n[2] + 1], s); c->prof_n[2]++; }
         const cudaError_t e = cudaStreamSynchronize(s);
         if (rc == TKHP_ECUDA && e == cudaSuccess) {
