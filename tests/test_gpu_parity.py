@@ -524,3 +524,43 @@ def test_stored_matrix_elements_flag_is_ignored_in_fp64():
     mu = np.random.default_rng(2).standard_normal((s.n_atoms, 3)) * 0.1
     _assert_close(P1.tmatvec(mu).cpu().numpy(), oracle.tmatvec(s, mu), 1e-11)
     P0.close(); P1.close()
+
+
+@pytest.mark.parametrize("precision", ["mixed", "fp64", "fixed"])
+@pytest.mark.parametrize("flags", ["persistent", "no_persistent"])
+def test_tiles_mode_solver_paths(flags, precision):
+    """Config 0 (box too small for the finer lists: TILES): the persistent cooperative solve kernel
+    (k_pcg_tiles) and the launch-per-matvec loop against the dense solution, with the oracle's
+    iteration counts, a converged guess and open-boundary input."""
+    pk = _pk()
+    s = SYSTEMS["cfg0"]()
+    prec = {"mixed": pk.TKHP_MIXED, "fp64": pk.TKHP_FP64, "fixed": pk.TKHP_FIXED}[precision]
+    P = pk.Polarizer.for_system(s, precision=prec, list_mode=pk.TKHP_LIST_ATOM,
+                                solver_flags=0 if flags == "persistent" else pk.TKHP_SOLVER_NO_PERSISTENT)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    assert P.nblist_stats(count_pairs=False)[2] == pk.TKHP_LIST_TILES
+    E_ref = oracle.perm_field(s)
+    mu_ref = oracle.dense_solve(s, E_ref)
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    tight = 1e-12 if precision == "fp64" else 1e-8
+    mu, it, rms = P.polar_solve(Eg, tol=tight)
+    assert rms < tight
+    _assert_close(mu.cpu().numpy(), mu_ref, 1e-10 if precision == "fp64" else 1e-5)
+    for tol in (1e-5, 1e-6):
+        _, it_ref, _ = oracle.pcg_solve(s, E_ref, tol=tol)
+        _, it_t, rms_t = P.polar_solve(Eg, tol=tol)
+        assert it_t == it_ref and rms_t < tol
+    _, it0, _ = P.polar_solve(Eg, tol=1e-6, guess=mu)
+    assert it0 == 0
+    e_ref = oracle.polar_energy(mu_ref, E_ref)
+    assert abs(float(P.polar_energy(mu, Eg).cpu()) - e_ref) <= 1e-6 * abs(e_ref)
+    P.close()
+    # open boundary, no Ewald: 200 random sites
+    s2 = tiny_cluster(200, 31, box=0.0, spread=14.0, group_size=1, cutoff=6.0, skin=1.0)
+    P2 = pk.Polarizer.for_system(s2, precision=prec, list_mode=pk.TKHP_LIST_TILES,
+                                 solver_flags=0 if flags == "persistent" else pk.TKHP_SOLVER_NO_PERSISTENT)
+    P2.nblist_build(s2.pos, s2.polarizability, s2.group_id)
+    E2 = oracle.perm_field(s2)
+    mu2, _, _ = P2.polar_solve(P2.perm_field(s2.charge, s2.dipole, s2.quad), tol=tight)
+    _assert_close(mu2.cpu().numpy(), oracle.dense_solve(s2, E2), 1e-10 if precision == "fp64" else 1e-5)
+    P2.close()
