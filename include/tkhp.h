@@ -96,7 +96,10 @@ typedef struct {
 
 /* tkhp_params.solver_flags */
 enum {
-    TKHP_SOLVER_NO_PERSISTENT = 1, /* never run the solve as one persistent cooperative kernel */
+    TKHP_SOLVER_NO_PERSISTENT = 1, /* never run the solve as one persistent cooperative kernel (k_pcg_persist: MIXED/
+                                      FIXED precision, ATOM lists, every group's neighbourhood in one chunk, grid
+                                      co-resident; k_pcg_tiles: TILES mode, at most 16,384 padded atoms, any
+                                      precision); the launch-per-matvec loop is used instead */
     TKHP_SOLVER_NO_FUSED_STEP = 2, /* launch-per-matvec path: update and direction as two kernels */
     TKHP_SOLVER_STORED_T = 4       /* MIXED/FIXED precision, ATOM lists: precompute the real-space matrix elements
                                       (two radial factors per list slot, 8 bytes) after a list build and stream
@@ -235,7 +238,7 @@ int tkhp_last_timings(tkhp_ctx *ctx, double ms[5]);
 int tkhp_profile_reset(tkhp_ctx *ctx, int32_t enable_kernel_events);
 int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmatvec_kernels,
                       double *tmatvec_kernel_ms, int32_t *n_field_kernels, double *field_kernel_ms);
-/* The same for the persistent PCG kernel (MIXED precision, ATOM lists: the whole solve is one
+/* The same for the persistent PCG kernels (k_pcg_persist, k_pcg_tiles: the whole solve is one
  * cooperative launch): recorded launches since the reset, their summed
  * duration in ms and the T.mu products they performed (iterations + 1 per solve). */
 int tkhp_profile_read_solve(tkhp_ctx *ctx, int32_t *n_solve_kernels, double *solve_kernel_ms, int64_t *n_matvecs);
