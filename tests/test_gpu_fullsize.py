@@ -288,3 +288,27 @@ def test_cfg2_fixed_point_mode(cfg2, cfg2_oracle):
     e_g = float(P.polar_energy(mu_g, Eg).cpu())
     assert abs(e_g - ref["e_pol"]) <= 1e-6 * abs(ref["e_pol"])
     P.close()
+
+
+def test_cfg2_stored_matrix_elements(cfg2, cfg2_oracle):
+    """TKHP_SOLVER_STORED_T at the headline size: the product with stored elements on
+    every row of config 2, and the solve that uses it (launch-per-matvec path), against the same oracle
+    results, at the MIXED bars."""
+    import paper_2011_01207_b200 as pk
+    s, ref = cfg2, cfg2_oracle
+    P = pk.Polarizer.for_system(s, precision=pk.TKHP_MIXED, list_mode=pk.TKHP_LIST_ATOM,
+                                solver_flags=pk.TKHP_SOLVER_STORED_T)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    n_pair, _, mode = P.nblist_stats()
+    assert mode == pk.TKHP_LIST_ATOM and n_pair == ref["n_pair"]
+    _assert_close(P.tmatvec(ref["probe"]).cpu().numpy(), ref["T"], 1e-5)
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    mu, _, rms = P.polar_solve(Eg, tol=1e-8)
+    assert rms < 1e-8
+    _assert_close(mu.cpu().numpy(), ref["mu"], 1e-5)
+    e_g = float(P.polar_energy(mu, Eg).cpu())
+    assert abs(e_g - ref["e_pol"]) <= 1e-6 * abs(ref["e_pol"])
+    _, it6, rms6 = P.polar_solve(Eg, tol=1e-6)
+    _, it_o, _ = oracle.pcg_solve(s, ref["E"], tol=1e-6)
+    assert it6 == it_o and rms6 < 1e-6
+    P.close()
