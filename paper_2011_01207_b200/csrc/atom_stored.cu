@@ -15,19 +15,9 @@
 // tkhp_tmatvec and the launch-per-matvec PCG path then use the stored product; the elements are
 // computed lazily by the first product after a list build and stay valid until the next build.
 #include "atom_tmu.cuh"
-#include "reduce.cuh"
+#include "atom_epilogue.cuh"
 
 namespace tkhp {
-
-// epilogue shared with atom_pairs.cu (q = p/alpha - T p - self p and p.q of the PCG loop)
-struct PcgFuseS {
-    int on;
-    double self;
-    const double *vp;
-    const double *inv_alpha;
-    double *vq;
-    double *part;
-};
 
 // ---- the two radial factors of one pair, scalar FP32 (the formulas of tmu_far2 / tmu_near2)
 __device__ __forceinline__ float2 radial_far(float s, const TmuConsts &K) {
@@ -180,7 +170,7 @@ __device__ __forceinline__ uint4 ldg_stream(const uint4 *p) {
 __global__ void __launch_bounds__(GT, 3)
 k_atom_tmu_stored(ClusterWs ws, const float4 *__restrict__ stage_pos, const float4 *__restrict__ mu,
                   const uint4 *__restrict__ tstore, double *__restrict__ acc, int n_pad, int s_chunk, int fixed,
-                  DeviceState *st, int iter, PcgFuseS fuse) {
+                  DeviceState *st, int iter, PcgFuse fuse) {
     if (iter >= 0 && iter >= st->conv_at) return;      // PCG already converged (pcg.cu)
     constexpr int SU = 4;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -277,40 +267,7 @@ k_atom_tmu_stored(ClusterWs ws, const float4 *__restrict__ stage_pos, const floa
     }
     A.flush(dx, dy, dz, fixed);
     dx = acc_value(dx, fixed != 0); dy = acc_value(dy, fixed != 0); dz = acc_value(dz, fixed != 0);
-    // ---- epilogue: parts of a shared block, result, and the PCG fusion (q, p.q)
-    if (wpb > 1) {
-        double *s_part = reinterpret_cast<double *>(smem_raw);
-        __syncthreads();
-        if (part > 0) { s_part[w * 96 + lane] = dx; s_part[w * 96 + 32 + lane] = dy; s_part[w * 96 + 64 + lane] = dz; }
-        __syncthreads();
-        if (part == 0)
-            for (int k = 1; k < wpb; ++k) {
-                dx += s_part[(w + k) * 96 + lane]; dy += s_part[(w + k) * 96 + 32 + lane]; dz += s_part[(w + k) * 96 + 64 + lane];
-            }
-    }
-    const bool owner = kb < nb && part == 0;
-    if (owner) {
-        acc[slot] = dx;
-        acc[n_pad + slot] = dy;
-        acc[2 * (size_t)n_pad + slot] = dz;
-    }
-    if (fuse.on) {
-        double pq = 0, dummy = 0;
-        if (owner) {
-            const double ia = fuse.inv_alpha[slot];
-            const double dd[3] = {dx, dy, dz};
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const size_t o = (size_t)k * n_pad + slot;
-                const double p = fuse.vp[o];
-                const double q = p * ia - dd[k] - fuse.self * p;
-                fuse.vq[o] = q;
-                pq += p * q;
-            }
-        }
-        block_sum2(pq, dummy);
-        if (grid_sum2_last_block(fuse.part, &st->ticket, pq, dummy) && threadIdx.x == 0) st->pq = pq;
-    }
+    pair_epilogue<true>(smem_raw, dx, dy, dz, wpb, part, kb < nb, slot, n_pad, acc, st, fuse);
 }
 
 // ----------------------------------------------------------------------------- host side
@@ -355,7 +312,7 @@ int atom_stored_tmatvec(Ctx *c, cudaStream_t s) {
         c->n_launches += 1;
         c->tstore_valid = true;
     }
-    PcgFuseS fuse;
+    PcgFuse fuse;
     fuse.on = c->fuse_q;
     const double b = c->p.ewald_beta;
     fuse.self = 4.0 * b * b * b / (3.0 * SQRT_PI);
