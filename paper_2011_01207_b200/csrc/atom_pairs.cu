@@ -136,7 +136,7 @@ __device__ __forceinline__ uint4 lds128(unsigned addr) {
 
 // resident CTAs per SM the register allocation must allow: FP32 field 2 (112 KB of staging), FP64 T.mu 2
 // (53 KB), FP64 field 1 (106 KB)
-template <typename real, int MODE> struct MinCtas { static constexpr int N = (sizeof(real) == 8 && MODE == MODE_FIELD) ? 1 : 2; };
+template <typename real, int MODE> struct MinCtas { static constexpr int N = (sizeof(real) == 8 && MODE == MODE_FIELD) ? 1 : (sizeof(real) == 8 ? 3 : 2); };
 
 // ----------------------------------------------------------------------------- generic kernel
 template <typename real, int MODE>
@@ -252,8 +252,14 @@ k_atom_pairs(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
 #pragma unroll
                         for (int k = 0; k < 4; ++k) {
                             if (k < n_here) {
-                                const unsigned o2[2] = {wd[k] & 0xffffu, wd[k] >> 16};
-                                eval_pairs<real, MODE, 2, THOLE>(s_base, pay_stride, o2, pi, gi, kc, A);
+                                if (sizeof(real) == 8 && MODE == MODE_TMU) {       // FP64 T.mu: one pair at a time (registers: 3 CTAs per SM)
+                                    const unsigned oa[1] = {wd[k] & 0xffffu}, ob[1] = {wd[k] >> 16};
+                                    eval_pairs<real, MODE, 1, THOLE>(s_base, pay_stride, oa, pi, gi, kc, A);
+                                    eval_pairs<real, MODE, 1, THOLE>(s_base, pay_stride, ob, pi, gi, kc, A);
+                                } else {
+                                    const unsigned o2[2] = {wd[k] & 0xffffu, wd[k] >> 16};
+                                    eval_pairs<real, MODE, 2, THOLE>(s_base, pay_stride, o2, pi, gi, kc, A);
+                                }
                             }
                         }
                         if (++since_flush == 4) {          // every 32 entries: FP32 partial -> 64-bit container
