@@ -390,7 +390,7 @@ void atom_far_setup(Ctx *c) {
     c->far_x0 = 0.0;
     c->far_rmin = 0.0;
     for (int k = 0; k < 6; ++k) c->far_q[k] = 0.f;
-    // (FP64 with a Thole-free first class, x >= 45, was measured: T.mu 0.191 -> 0.213 ms on config 2; not used)
+    // (FP64 with a Thole-free first class, x >= 45, was measured twice: T.mu 0.191 -> 0.213 ms and, with the 3-CTA kernel, 0.181 -> 0.190 ms on config 2; not used)
     if (c->p.precision == TKHP_FP64 || !(beta > 0.0) || z_max < 1.25 * z_min) return;    // no far class: full formula everywhere
     c->far_on = true;
     constexpr int D = 5;
