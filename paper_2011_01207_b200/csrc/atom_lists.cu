@@ -33,35 +33,54 @@ namespace tkhp {
 // access): k_atom_lists is bound by its instruction count.
 struct Deal {
     uint8_t *cnt;      // this lane's counters: cnt[b * 32], b = 0..15
-    int k = 0;
+    int novf = 0;      // entries on the overflow stack (top rows of the image)
     __device__ __forceinline__ void clear() {
 #pragma unroll
         for (int b = 0; b < 16; ++b) cnt[b * 32] = 0;
-        k = 0;
+        novf = 0;
     }
 };
-
-// put one entry into the image; a full column spills into the next one (only a bank conflict later)
-__device__ __forceinline__ void deal(Deal &d, uint16_t *img, int colcap, unsigned l16, unsigned off, unsigned bank) {
-    unsigned b = bank, r = d.cnt[b * 32];
-    while (r >= (unsigned)colcap) {
-        b = (b + 1) & 15u;
-        r = d.cnt[b * 32];
-    }
-    const unsigned t = ((b - l16) & 15u) + 16u * r;
-    img[t * 32] = (uint16_t)off;
-    d.cnt[b * 32] = (uint8_t)(r + 1);
-    ++d.k;
-}
 
 // rows of column j that lie inside a list of `len` entries
 __device__ __forceinline__ unsigned col_cap(unsigned j, unsigned len) { return j < len ? (len - j + 15u) >> 4 : 0u; }
 
-// Entries of over-full columns -> holes of under-full ones (per lane, no cross-lane traffic).  First
-// into the PARTNER column (j + 8) mod 16: its steps want the same index class mod 8, so the quarter
-// warp's LDS.128 stays conflict-free and only the half warp's LDS.64 takes a second wavefront; what
-// is left goes into any hole (those steps may conflict with one other lane).
-__device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16, unsigned len) {
+// Put one entry into the image: into its own column, or, when that column is full, onto the overflow
+// stack that grows down from row `top` of the image (branch-free: this pass is bound by its instruction
+// stream, and a probing loop runs as long as its slowest lane).  The stack has `ovf_cap` cells above
+// the rows the class can use; an entry that finds it full probes the next columns (rare).
+__device__ __forceinline__ void deal(Deal &d, uint16_t *img, int colcap, unsigned l16, unsigned off, unsigned bank,
+                                     int top, int ovf_cap) {
+    unsigned b = bank, r = d.cnt[b * 32];
+    bool ok = r < (unsigned)colcap;
+    if (!ok && d.novf >= ovf_cap) {
+        do {
+            b = (b + 1) & 15u;
+            r = d.cnt[b * 32];
+        } while (r >= (unsigned)colcap);
+        ok = true;
+    }
+    const unsigned t = ok ? ((b - l16) & 15u) + 16u * r : (unsigned)(top - d.novf);
+    img[t * 32] = (uint16_t)off;
+    d.cnt[b * 32] = (uint8_t)(r + (ok ? 1u : 0u));
+    d.novf += ok ? 0 : 1;
+}
+
+// the next hole of the image in column order (there is one: the class is padded to its longest lane)
+__device__ __forceinline__ void to_hole(const Deal &d, uint16_t *img, unsigned l16, unsigned len, unsigned &hb, uint16_t v) {
+    unsigned hr = d.cnt[hb * 32];
+    while (hr >= col_cap((hb - l16) & 15u, len)) {
+        ++hb;
+        hr = d.cnt[hb * 32];
+    }
+    img[(((hb - l16) & 15u) + 16u * hr) * 32] = v;
+    d.cnt[hb * 32] = (uint8_t)(hr + 1);
+}
+
+// Entries of over-full columns and of the overflow stack -> holes of under-full columns (per lane, no
+// cross-lane traffic).  First into the PARTNER column (j + 8) mod 16: its steps want the same index
+// class mod 8, so the quarter warp's LDS.128 stays conflict-free and only the half warp's LDS.64 takes
+// a second wavefront; what is left goes into any hole (those steps may conflict with one other lane).
+__device__ __forceinline__ void level(Deal &d, uint16_t *img, unsigned l16, unsigned len, int top, unsigned rec_shift) {
     // pass 1: partner columns
     for (unsigned b = 0; b < 16; ++b) {
         const unsigned j = (b - l16) & 15u, pb = (b + 8u) & 15u, pj = (pb - l16) & 15u;
@@ -77,18 +96,23 @@ __device__ __forceinline__ void level(const Deal &d, uint16_t *img, unsigned l16
         d.cnt[pb * 32] = (uint8_t)cp;
     }
     // pass 2: whatever is still over the edge, into the holes in column order
-    unsigned hb = 0, hr = d.cnt[0];
+    unsigned hb = 0;
     for (unsigned b = 0; b < 16; ++b) {
         const unsigned j = (b - l16) & 15u;
         const unsigned cb = d.cnt[b * 32];
-        for (unsigned r = col_cap(j, len); r < cb; ++r) {
-            const uint16_t v = img[(j + 16u * r) * 32];
-            while (hr >= col_cap((hb - l16) & 15u, len)) {
-                ++hb;
-                hr = d.cnt[hb * 32];
-            }
-            img[(((hb - l16) & 15u) + 16u * hr) * 32] = v;
-            ++hr;
+        for (unsigned r = col_cap(j, len); r < cb; ++r) to_hole(d, img, l16, len, hb, img[(j + 16u * r) * 32]);
+    }
+    // pass 3: the overflow stack, partner column first
+    for (int i = 0; i < d.novf; ++i) {
+        const uint16_t v = img[(top - i) * 32];
+        img[(top - i) * 32] = 0xffffu;
+        const unsigned pb = (((unsigned)v >> rec_shift) + 8u) & 15u, pj = (pb - l16) & 15u;
+        const unsigned cp = d.cnt[pb * 32];
+        if (cp < col_cap(pj, len)) {
+            img[(pj + 16u * cp) * 32] = v;
+            d.cnt[pb * 32] = (uint8_t)(cp + 1);
+        } else {
+            to_hole(d, img, l16, len, hb, v);
         }
     }
 }
@@ -287,6 +311,9 @@ k_atom_deal(ClusterWs ws, int n_blocks, int rec_bytes) {
             r0 += nrow;
             if (nrow == 0 || 8 * nrow > img_rows) continue;          // (an over-long class keeps its arrival order)
             const int colcap = (8 * nrow + 15) >> 4;
+            const int top = img_rows - 1;
+            int ovf_cap = img_rows - 16 * colcap;                    // free rows above the cells the class can use
+            if (ovf_cap < 0) ovf_cap = 0;
             uint4 nxt = p[0];
             for (int q = 0; q < nrow; ++q) {
                 const uint4 e = nxt;
@@ -295,9 +322,9 @@ k_atom_deal(ClusterWs ws, int n_blocks, int rec_bytes) {
                                        e.z & 0xffffu, e.z >> 16, e.w & 0xffffu, e.w >> 16};
 #pragma unroll
                 for (int h = 0; h < 8; ++h)
-                    if (v[h] < dummy) deal(D, img, colcap, l16, v[h], (v[h] >> rec_shift) & 15u);      // (the scan pads with the first dummy)
+                    if (v[h] < dummy) deal(D, img, colcap, l16, v[h], (v[h] >> rec_shift) & 15u, top, ovf_cap);      // (the scan pads with the first dummy)
             }
-            level(D, img, l16, (unsigned)len);
+            level(D, img, l16, (unsigned)len, top, rec_shift);
             for (int q = 0; q < nrow; ++q) {
                 unsigned v[8];
 #pragma unroll
