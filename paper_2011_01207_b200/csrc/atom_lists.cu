@@ -172,8 +172,14 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     // this lane's far row fw / 8 of the open segment from the ring; entries from `valid` on are padding
     auto put_row = [&](int valid) {
         unsigned v[8];
+        const uint16_t *q8 = fq + (fw & (FQ - 1)) * 32;          // fw is a multiple of 8: the row's entries are q8[h * 32]
+        if (valid - fw >= 8) {                                   // (the usual call: a whole row is waiting)
 #pragma unroll
-        for (int h = 0; h < 8; ++h) v[h] = fw + h < valid ? fq[((fw + h) & (FQ - 1)) * 32] : dummy;
+            for (int h = 0; h < 8; ++h) v[h] = q8[h * 32];
+        } else {
+#pragma unroll
+            for (int h = 0; h < 8; ++h) v[h] = fw + h < valid ? q8[h * 32] : dummy;
+        }
         const int r = row_cur + (fw >> 3);
         if (r < rows_cap) rows[(size_t)r * 32] = make_uint4(v[0] | (v[1] << 16), v[2] | (v[3] << 16), v[4] | (v[5] << 16), v[6] | (v[7] << 16));
         fw += 8;
@@ -236,7 +242,7 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
                 const unsigned loc = ONE ? e : (e * magic) >> 20;              // e / n_chunks
                 bool hit = (int)e < count && (ONE || e - loc * (unsigned)n_chunks == (unsigned)c);   // padding entries are == count
                 if (h == 7) open = (int)e < count;                             // padding only at the end of a list
-                const vec4 pj = s_pos[hit ? loc : 0u];
+                const vec4 pj = s_pos[loc];                                    // (a padding entry reads one record past the chunk: inside the shared-memory block, and hit is false)
                 const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
                 const real r2 = Rx * Rx + Ry * Ry + Rz * Rz;
                 hit = hit && r2 <= rc2 && r2 > (real)1e-10;
