@@ -159,7 +159,7 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
     uint4 *__restrict__ rows = reinterpret_cast<uint4 *>(ws.alist + (size_t)blk * ws.a_cap * 32) + lane;    // row r of this lane: rows[r * 32]
     const int rows_cap = ws.a_cap >> 3;
     const int fcap = ws.far_cap;
-    uint16_t *nbuf = reinterpret_cast<uint16_t *>(smem_raw + (size_t)s_chunk * sizeof(vec4)) +
+    uint16_t *nbuf = reinterpret_cast<uint16_t *>(smem_raw + (size_t)(s_chunk + 1) * sizeof(vec4)) +
                      (size_t)w * (NEAR_CAP + FQ) * 32 + lane;                            // nbuf[k * 32]
     uint16_t *fq = nbuf + NEAR_CAP * 32;                                                 // fq[(k & 15) * 32]
 
@@ -240,7 +240,8 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             for (int h = 0; h < 8; ++h) {
                 const unsigned e = (word[h >> 1] >> ((h & 1) * 16)) & 0xffffu;
                 const unsigned loc = ONE ? e : (e * magic) >> 20;              // e / n_chunks
-                bool hit = (int)e < count && (ONE || e - loc * (unsigned)n_chunks == (unsigned)c);   // padding entries are == count
+                // padding entries are == count: ONE: they read the far record behind the chunk, no test needed
+                bool hit = ONE || ((int)e < count && e - loc * (unsigned)n_chunks == (unsigned)c);
                 if (h == 7) open = (int)e < count;                             // padding only at the end of a list
                 const vec4 pj = s_pos[loc];                                    // (a padding entry reads one record past the chunk: inside the shared-memory block, and hit is false)
                 const real Rx = pi.x - pj.x, Ry = pi.y - pj.y, Rz = pi.z - pj.z;
@@ -267,6 +268,11 @@ k_atom_scan(ClusterWs ws, const typename Vec4<real>::type *__restrict__ gpos,
             vec4 p = stage_pos[gbase + idx];
             p.w = cbrt(p.w * p.w);                       // the class test wants w^(2/3)
             s_pos[l] = p;
+        }
+        if (t == 0 && n_chunks == 1) {                   // the record the padding entries (== count) point at: far away
+            vec4 far;
+            far.x = far.y = far.z = (real)(-3.0f * PHANTOM_FAR); far.w = 0;
+            s_pos[count] = far;
         }
         __syncthreads();
         if (!active) continue;
@@ -361,7 +367,7 @@ int atom_build(Ctx *c, cudaStream_t s) {
     ClusterWs ws = get_ws(c);
     const bool f64 = c->p.precision == TKHP_FP64;
     const int s_chunk = atom_chunk_capacity(f64, ws.chunk_cap);
-    const size_t smem = (size_t)s_chunk * (f64 ? sizeof(double4) : sizeof(float4)) + (size_t)GB * (NEAR_CAP + FQ) * 32 * sizeof(uint16_t);
+    const size_t smem = (size_t)(s_chunk + 1) * (f64 ? sizeof(double4) : sizeof(float4)) + (size_t)GB * (NEAR_CAP + FQ) * 32 * sizeof(uint16_t);
     const double rc2 = c->p.cutoff * c->p.cutoff;
     // far class off (FP64, beta = 0): far_r2 < 0 puts every pair into the first class of rows, which
     // the kernels then evaluate with the full formula
