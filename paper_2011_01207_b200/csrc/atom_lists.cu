@@ -42,7 +42,7 @@ struct Deal {
 };
 
 // rows of column j that lie inside a list of `len` entries
-__device__ __forceinline__ unsigned col_cap(unsigned j, unsigned len) { return j < len ? (len - j + 15u) >> 4 : 0u; }
+__device__ __forceinline__ unsigned col_cap(unsigned j, unsigned len) { return (len + 15u - j) >> 4; }     // (0 for j >= len: j <= 15)
 
 // Put one entry into the image: into its own column, or, when that column is full, onto the overflow
 // stack that grows down from row `top` of the image (branch-free: this pass is bound by its instruction
