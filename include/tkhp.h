@@ -118,7 +118,8 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
 int tkhp_destroy(tkhp_ctx *ctx);
 
 /* Text of the last error on this context (ctx-owned, valid until the next call);
- * with ctx == NULL: the last error of a failed tkhp_create() on this thread. */
+ * with ctx == NULL: the last error of a failed tkhp_create() (or of a context-free call such as
+ * tkhp_polar_energy_static) on this thread. */
 const char *tkhp_last_error(const tkhp_ctx *ctx);
 
 /*
@@ -205,6 +206,46 @@ int tkhp_polar_solve(tkhp_ctx *ctx, const double *d_field, double *d_mu, double 
 /* *d_energy (device, 1 double) = -1/2 * 332.063713 * sum_i mu_i . field_i  (kcal/mol). */
 int tkhp_polar_energy(tkhp_ctx *ctx, const double *d_mu, const double *d_field,
                       double *d_energy, void *stream);
+
+/*
+ * The same energy for callers that cannot allocate: no context, no workspace, no cudaMalloc.
+ *
+ * Who this is for.  Every other call needs a tkhp_ctx, and tkhp_create() needs a workspace that
+ * somebody obtained from cudaMalloc (it also creates streams, events and pinned host buffers).
+ * Code that runs where allocation is off limits cannot provide that: a force-field plug-in called
+ * from inside an MD engine's step loop after the engine has given all device memory to its own
+ * pool; a callback that runs while another host thread has a stream capture open, when the CUDA
+ * runtime refuses cudaMalloc; a step loop that cannot afford the device-wide stall of
+ * cudaMalloc/cudaFree.  Such a caller already holds mu and the field on the device and wants
+ * E_pol = -1/2 * 332.063713 * sum_i mu_i . field_i in *d_energy (device, 1 double, kcal/mol).
+ *
+ *   device    CUDA device ordinal that owns d_mu, d_field, d_energy and `stream` (0..63)
+ *   n_atoms   1 <= n_atoms <= TKHP_STATIC_MAX_ATOMS; d_mu, d_field: n_atoms*3 FP64, any atom order
+ *
+ * The block partial sums and the ticket counter of the reduction live in an 8,448-byte array that is
+ * part of the library's device image (a file-scope __device__ array in csrc/energy_static.cu): every
+ * GPU that loads libtkhp holds these bytes until the process exits, and this call neither creates nor
+ * frees anything -- it calls no cudaMalloc, cudaFree, cudaHostAlloc or allocating library routine.
+ * The scratch is sized for 1,024 partial sums; beyond TKHP_STATIC_MAX_ATOMS (2^22, four times the
+ * paper's largest system) the call is refused with TKHP_ECAPACITY and leaves *d_energy untouched.
+ *
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, which also makes
+ * the CUDA runtime load the library's device code on that GPU).  That is host-side set-up, done once
+ * per device under a mutex; make this first call before you begin any stream capture.
+ *
+ * Sharing: all calls on a GPU use the same array, which keeps whatever the previous call left.  The
+ * call clears the ticket on `stream` before the kernel; the partials need no clearing.  Two calls
+ * that can overlap on the GPU (different streams without an ordering between them, or different host
+ * threads on the same device) race on the array and give wrong energies: order them.
+ *
+ * Asynchronous on `stream`; leaves the caller's current device as it found it.  The value is that of
+ * tkhp_polar_energy on an FP64 or MIXED context, same summation order (TKHP_FIXED contexts round every
+ * term to 2^-30 kcal/mol first; this call does not).  Errors: TKHP_EINVAL (NULL pointer, n_atoms < 1,
+ * device ordinal), TKHP_ECAPACITY (n_atoms too large), TKHP_ECUDA; tkhp_last_error(NULL) has the text.
+ */
+#define TKHP_STATIC_MAX_ATOMS 4194304
+int tkhp_polar_energy_static(int32_t device, int64_t n_atoms, const double *d_mu, const double *d_field,
+                             double *d_energy, void *stream);
 
 /*
  * Whole hot path from HOST buffers (end-to-end entry used for the e2e benchmark leg):

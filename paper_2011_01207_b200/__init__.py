@@ -15,7 +15,8 @@ from .binding import (TKHP_FP64, TKHP_MIXED, TKHP_FIXED, TKHP_LIST_TILES, TKHP_L
                       tkhp_workspace_bytes, tkhp_create, tkhp_destroy, tkhp_last_error,
                       tkhp_nblist_build, tkhp_nblist_view, tkhp_nblist_stats, tkhp_nblist_atom_stats,
                       tkhp_perm_field, tkhp_tmatvec, tkhp_polar_solve,
-                      tkhp_polar_energy, tkhp_polarize_host, tkhp_last_timings,
+                      tkhp_polar_energy, tkhp_polar_energy_static, TKHP_STATIC_MAX_ATOMS,
+                      tkhp_polarize_host, tkhp_last_timings,
                       tkhp_fma_peak, tkhp_profile_reset, tkhp_profile_read, tkhp_profile_read_solve,
                       EXPORTED_SYMBOLS)
 
@@ -24,6 +25,6 @@ __all__ = [
     "TkhpParams", "Polarizer", "lib", "lib_path", "tkhp_workspace_bytes", "tkhp_create",
     "tkhp_destroy", "tkhp_last_error", "tkhp_nblist_build", "tkhp_nblist_view",
     "tkhp_nblist_stats", "tkhp_nblist_atom_stats", "tkhp_perm_field", "tkhp_tmatvec", "tkhp_polar_solve",
-    "tkhp_polar_energy", "tkhp_polarize_host", "tkhp_last_timings", "tkhp_fma_peak",
+    "tkhp_polar_energy", "tkhp_polar_energy_static", "TKHP_STATIC_MAX_ATOMS", "tkhp_polarize_host", "tkhp_last_timings", "tkhp_fma_peak",
     "tkhp_profile_reset", "tkhp_profile_read", "tkhp_profile_read_solve", "EXPORTED_SYMBOLS",
 ]

@@ -12,6 +12,7 @@ TKHP_ENOCONV, TKHP_ECAPACITY, TKHP_ENONFINITE = -5, -6, -7
 TKHP_FP64, TKHP_MIXED, TKHP_FIXED = 0, 1, 2
 TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM = 0, 1, 2
 TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP, TKHP_SOLVER_STORED_T = 1, 2, 4
+TKHP_STATIC_MAX_ATOMS = 4194304
 
 _ERR_NAMES = {-1: "TKHP_EINVAL", -2: "TKHP_ECUDA", -3: "TKHP_ECUTOFF", -4: "TKHP_ENOLIST",
               -5: "TKHP_ENOCONV", -6: "TKHP_ECAPACITY", -7: "TKHP_ENONFINITE"}
@@ -19,7 +20,7 @@ _ERR_NAMES = {-1: "TKHP_EINVAL", -2: "TKHP_ECUDA", -3: "TKHP_ECUTOFF", -4: "TKHP
 EXPORTED_SYMBOLS = [
     "tkhp_workspace_bytes", "tkhp_create", "tkhp_destroy", "tkhp_last_error",
     "tkhp_nblist_build", "tkhp_nblist_view", "tkhp_nblist_stats", "tkhp_nblist_atom_stats", "tkhp_perm_field",
-    "tkhp_tmatvec", "tkhp_polar_solve", "tkhp_polar_energy", "tkhp_polarize_host",
+    "tkhp_tmatvec", "tkhp_polar_solve", "tkhp_polar_energy", "tkhp_polar_energy_static", "tkhp_polarize_host",
     "tkhp_last_timings", "tkhp_fma_peak", "tkhp_profile_reset", "tkhp_profile_read",
     "tkhp_profile_read_solve",
 ]
@@ -75,6 +76,7 @@ def lib() -> ctypes.CDLL:
         L.tkhp_polar_solve.argtypes = [c_void_p, dp, dp, c_double, c_int32, c_int32,
                                        POINTER(c_int32), POINTER(c_double), vp]
         L.tkhp_polar_energy.argtypes = [c_void_p, dp, dp, dp, vp]
+        L.tkhp_polar_energy_static.argtypes = [c_int32, c_int64, dp, dp, dp, vp]
         L.tkhp_polarize_host.argtypes = [c_void_p, vp, vp, vp, vp, vp, vp, c_double, c_int32,
                                          vp, vp, vp, POINTER(c_int32), POINTER(c_double), vp]
         L.tkhp_last_timings.argtypes = [c_void_p, POINTER(c_double)]
@@ -189,6 +191,20 @@ def tkhp_polar_solve(ctx, d_field, d_mu, tol=1e-6, max_iter=100, use_guess=False
 def tkhp_polar_energy(ctx, d_mu, d_field, d_energy, stream=None):
     _check(lib().tkhp_polar_energy(ctx, _ptr(d_mu), _ptr(d_field), _ptr(d_energy),
                                    _stream_ptr(stream)), ctx)
+
+
+def tkhp_polar_energy_static(device: int, n_atoms: int, d_mu, d_field, d_energy, stream=None):
+    """E_pol into ``d_energy`` without a context or a workspace, for code that may not allocate
+    device memory (a plug-in inside an MD engine's step loop whose memory all belongs to the
+    engine's pool, a callback running while a stream capture is open elsewhere, a loop that
+    cannot take cudaMalloc's device-wide stall).  The reduction's scratch is a fixed 8,448-byte
+    array inside libtkhp's device image; ``n_atoms`` may be at most ``TKHP_STATIC_MAX_ATOMS``.
+    Calls on one GPU share that array: do not let two of them overlap.  See include/tkhp.h."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream(device)
+    _check(lib().tkhp_polar_energy_static(device, n_atoms, _ptr(d_mu), _ptr(d_field), _ptr(d_energy),
+                                          _stream_ptr(stream)))
 
 
 def tkhp_polarize_host(ctx, h_pos, h_polarizability, h_group_id, h_charge, h_dipole, h_quad,

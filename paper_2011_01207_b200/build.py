@@ -17,7 +17,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 OBJ = PKG / "build"
 LIB = PKG / "libtkhp.so"
-SOURCES = ["api.cu", "nblist.cu", "tiles.cu", "cluster_build.cu", "cluster_pairs.cu", "atom_lists.cu", "atom_pairs.cu", "atom_solve.cu", "atom_stored.cu", "pcg.cu", "fma_peak.cu"]
+SOURCES = ["api.cu", "nblist.cu", "tiles.cu", "cluster_build.cu", "cluster_pairs.cu", "atom_lists.cu", "atom_pairs.cu", "atom_solve.cu", "atom_stored.cu", "pcg.cu", "fma_peak.cu", "energy_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false"]
 

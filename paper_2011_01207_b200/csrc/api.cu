@@ -9,6 +9,9 @@ namespace tkhp {
 
 static thread_local char g_create_err[512] = "";
 
+// for the entry points that have no context (energy_static.cu): the text tkhp_last_error(NULL) returns
+void set_thread_error(const char *msg) { snprintf(g_create_err, sizeof(g_create_err), "%s", msg); }
+
 static int grid_bits_for(double extent) {
     int b = 1;
     while (extent / (double)(1 << b) > 2.5 && b < 8) ++b;
