@@ -50,6 +50,39 @@ def test_wrap_and_cells():
         assert oracle.lib().oracle_wrap(float(v), L) == oracle.wrap(np.array([v]), L)[0]
 
 
+def test_open_boundary_cells_wide_system():
+    """Open-boundary branch of cell_coords (Q14) on a system wider than
+    2^6 x 2.5 A, where the OPEN_MAX_BITS cap decides the grid: origin = per-axis minimum, one
+    extent for all axes = 1.000001 * (largest axis span) + 1e-9, 64 cells per axis.  The expected
+    cells are written out by hand for atoms placed at known fractions of the extent."""
+    span = 400.0                                     # > 64 * 2.5 = 160 A: uncapped, grid_bits would give 8
+    extent = span * 1.000001 + 1e-9
+    assert oracle.grid_bits(extent) == 8 and oracle.OPEN_MAX_BITS == 6
+    h = extent / 64.0                                # cell edge of the capped grid, 6.25 A
+    origin = np.array([-123.0, 7.5, 1000.0])         # an open system sits anywhere
+    frac_cells = np.array([[0, 0, 0],                # the three per-axis minima
+                           [63, 0, 0],               # x = origin + span: last cell, not 64 (the 1.000001 margin)
+                           [0, 31, 0], [0, 32, 0],   # either side of the middle of y
+                           [10, 20, 30], [5, 63, 1]])
+    pos = origin[None, :] + (frac_cells + 0.5) * h
+    pos[0] = origin                                  # exactly on the minimum corner
+    pos[1, 0] = origin[0] + span                     # the maximum of the widest axis defines the extent
+    pos[5, 1] = origin[1] + 63.25 * h                # y and z spans are shorter than x's: same h on every axis
+    cells, b = oracle.cell_coords(pos, 0.0)
+    assert b == 6
+    np.testing.assert_array_equal(cells, frac_cells)
+    # coarser cells, same rule: a translation of the whole system changes no cell
+    cells2, b2 = oracle.cell_coords(pos + np.array([1e3, -2e3, 5.0]), 0.0)
+    assert b2 == 6
+    np.testing.assert_array_equal(cells2, frac_cells)
+    # narrower than 160 A the cap is idle: 100 A -> 2^6 cells of 1.5625 A by grid_bits itself, 30 A -> 2^4
+    small = np.array([[0.0, 0.0, 0.0], [100.0, 50.0, 25.0]])
+    c3, b3 = oracle.cell_coords(small, -1.0)
+    assert b3 == 6 and c3[1].tolist() == [63, 31, 15]
+    c4, b4 = oracle.cell_coords(small * 0.3, 0.0)
+    assert b4 == 4 and c4[1].tolist() == [15, 7, 3]
+
+
 def _sorted_perm(s):
     key = oracle.sort_keys(s.pos, s.box)
     order = np.lexsort((np.arange(s.n_atoms), key))
