@@ -19,8 +19,9 @@
 //    argument mapping: G1 and G2 come from t = 1/R, e^{-z^2} and one degree-5 polynomial, 2 MUFU and
 //    28 FMA-pipe cycles per pair instead of 4 and 40;
 //  * the FP32 T.mu kernel (k_atom_tmu32) evaluates two list entries per lane and call as the two
-//    halves of packed FP32 instructions (f32x2.cuh), streams the list rows through a per-warp
-//    shared-memory ring with cp.async, and keeps the staged records as (x, y, z, mu_z), (mu_x, mu_y)
+//    halves of packed FP32 instructions (f32x2.cuh), loads each list row from L2 into registers two
+//    rows before its use (RowStream in atom_tmu.cuh; the cp.async list ring of round 1 was measured and
+//    removed), and keeps the staged records as (x, y, z, mu_z), (mu_x, mu_y)
 //    and w: a far pair reads 24 bytes of shared memory;
 //  * a group with fewer than 5 blocks gives every block to 2, 4 or 8 warps (interleaved list rows);
 //  * FP32 partial sums are flushed into FP64 registers every 4 rows.
@@ -72,8 +73,8 @@ __device__ __forceinline__ void eval_pairs(const unsigned char *s_base, int pay_
     real &ax = A.x, &ay = A.y, &az = A.z;
     vec4 pj[W];
     real Rx[W], Ry[W], Rz[W], r2[W], ww[W], G[W][NK];
-#pragma unroll
     const int half = pay_stride >> 1;
+#pragma unroll
     for (int u = 0; u < W; ++u) pj[u] = RecLoad<real>::get(s_base, half, off[u]);
     if (MODE == MODE_TMU) {
         vec4 mj[W];
@@ -134,8 +135,8 @@ __device__ __forceinline__ uint4 lds128(unsigned addr) {
     return v;
 }
 
-// resident CTAs per SM the register allocation must allow: FP32 field 2 (112 KB of staging), FP64 T.mu 2
-// (53 KB), FP64 field 1 (106 KB)
+// resident CTAs per SM the register allocation must allow: FP32 field 2 (112 KB of staging), FP64 T.mu 3
+// (80 registers, 53 KB), FP64 field 1 (106 KB)
 template <typename real, int MODE> struct MinCtas { static constexpr int N = (sizeof(real) == 8 && MODE == MODE_FIELD) ? 1 : (sizeof(real) == 8 ? 3 : 2); };
 
 // ----------------------------------------------------------------------------- generic kernel

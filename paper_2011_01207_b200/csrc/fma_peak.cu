@@ -19,12 +19,23 @@ __global__ void __launch_bounds__(256) k_fma_chain(real *out, int iters, real a,
     if (s == (real)123456.789) out[0] = s;   // never true: keeps the chain alive
 }
 
+// the caller's current device is put back on every return path
+struct PeakDeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit PeakDeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        ok = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~PeakDeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 template <typename real>
 static int run_peak(int device, double seconds, double *tflops) {
     cudaDeviceProp prop;
-    if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess)
-        return TKHP_ECUDA;
-    real *out = nullptr;
+    PeakDeviceGuard guard(device);
+    if (!guard.ok || cudaGetDeviceProperties(&prop, device) != cudaSuccess) { cudaGetLastError(); return TKHP_ECUDA; }
+    real *out = nullptr;   // one scalar the chain never writes (this benchmark call allocates; see tkhp.h)
     if (cudaMalloc(&out, sizeof(real)) != cudaSuccess) return TKHP_ECUDA;
     const int ctas = prop.multiProcessorCount * 8;   // 8 x 256 threads = 2048 threads per SM
     const int iters = 4096;
@@ -38,7 +49,11 @@ static int run_peak(int device, double seconds, double *tflops) {
         cudaEventRecord(e0);
         for (int r = 0; r < 8; ++r) k_fma_chain<real><<<ctas, 256>>>(out, iters, (real)0.999, (real)0.001);
         cudaEventRecord(e1);
-        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(out); return TKHP_ECUDA; }
+        if (cudaEventSynchronize(e1) != cudaSuccess) {
+            cudaEventDestroy(e0); cudaEventDestroy(e1);
+            cudaFree(out);
+            return TKHP_ECUDA;
+        }
         float ms = 0;
         cudaEventElapsedTime(&ms, e0, e1);
         elapsed += ms * 1e-3;
