@@ -36,6 +36,7 @@ __all__ = [
     "polar_energy", "COULOMB", "wrap", "grid_bits", "cell_coords",
     "hilbert_key", "sort_keys", "check_perm", "block_boxes", "block_pairs",
     "atom_pairs_covered", "num_threads", "to_fixed", "from_fixed", "FIX_VEC_BITS", "FIX_ENERGY_BITS",
+    "polar_energy_fixed",
     "OPEN_MAX_BITS",
 ]
 
@@ -279,6 +280,17 @@ def to_fixed(x, frac_bits: int) -> np.ndarray:
 def from_fixed(a, frac_bits: int) -> np.ndarray:
     """Paper eq. (3): x = real(a) / 2^fB."""
     return np.asarray(a, dtype=np.int64).astype(np.float64) / float(1 << frac_bits)
+
+
+def polar_energy_fixed(mu, E) -> float:
+    """Paper's FP mode for the energy (Q21): every ATOM's term
+    -1/2 f mu_i . E_i is converted with eq. (2) at 30 fractional bits, the int64 terms are summed
+    (exactly, in any order) and the sum is converted back with eq. (3).  The dot product is
+    ((mu_x E_x + mu_y E_y) + mu_z E_z) in FP64 without fused multiply-adds, then times -f/2."""
+    mu, E = _f64(mu), _f64(E)
+    dot = (mu[:, 0] * E[:, 0] + mu[:, 1] * E[:, 1]) + mu[:, 2] * E[:, 2]
+    terms = to_fixed(dot * (-0.5 * COULOMB), FIX_ENERGY_BITS)
+    return float(from_fixed(int(terms.sum()), FIX_ENERGY_BITS))
 
 
 # ------------------------------------------------------------------ N

@@ -150,3 +150,40 @@ def test_fixed_point_containers_eqs_2_and_3():
     # integer sums are order independent (what makes the mode deterministic)
     a = o.to_fixed(rng.standard_normal(4096) * 1e-3, 34)
     assert int(a.sum()) == int(a[::-1].sum()) == int(np.sort(a).sum())
+
+
+def test_fixed_point_energy_converts_one_term_per_atom():
+    """polar_energy_fixed (Q21): the sum of per-atom terms rounded to 2^-30 kcal/mol.  Pins:
+    a hand-made case whose terms are exact multiples of 2^-30 (nothing is rounded: equals -1/2 f sum mu.E
+    computed in exact rational arithmetic); a term of 0.4 units rounds to 0 PER ATOM (three components of
+    0.4 units each would round to 0 + 0 + 0 = 0 as well, but 1.2 units per atom must give 1: this is what
+    separates per-atom from per-component conversion); the distance to the FP64 energy is at most half a
+    unit per atom; the value does not depend on the order of the atoms."""
+    import oracle as o
+    from fractions import Fraction
+    unit = 2.0 ** -30
+    f = Fraction(o.COULOMB)                                  # the double, exactly
+    # two atoms with mu.E = 1 exactly (the other components multiply zeros): two equal terms, each the integer
+    # nearest to -f/2 x 2^30, found here in rational arithmetic from the bits of the double f
+    mu = np.array([[2.0, 0.0, 0.0], [0.0, 4.0, 0.0]])
+    E = np.array([[0.5, 9.0, 9.0], [7.0, 0.25, 7.0]])       # dots: 1.0 and 1.0
+    exact_units = -f / 2 * 2 ** 30
+    nearest = int(exact_units - Fraction(1, 2)) if exact_units < 0 else int(exact_units + Fraction(1, 2))
+    assert abs(Fraction(nearest) - exact_units) < Fraction(1, 2)                 # no tie: the nearest integer is unique
+    want = Fraction(2 * nearest, 2 ** 30)
+    assert Fraction(o.polar_energy_fixed(mu, E)) == want
+    # per-atom, not per-component: each component contributes 0.4 units, the atom 1.2 units -> 1 unit
+    c = 0.4 * unit / (0.5 * o.COULOMB)                       # |mu_k E_k| worth 0.4 units of energy
+    mu1 = np.full((5, 3), 1.0)
+    E1 = np.full((5, 3), -c)                                 # energy term +1.2 units per atom
+    got = o.polar_energy_fixed(mu1, E1)
+    assert got == 5 * unit                                   # per-component rounding would give 0
+    # half a unit per atom at most, and order independence
+    rng = np.random.default_rng(11)
+    mu2 = rng.standard_normal((777, 3)) * 0.05
+    E2 = rng.standard_normal((777, 3)) * 0.1
+    e_fix = o.polar_energy_fixed(mu2, E2)
+    assert abs(e_fix - o.polar_energy(mu2, E2)) <= 777 * 0.5 * unit + 1e-12
+    assert e_fix * 2.0 ** 30 == np.rint(e_fix * 2.0 ** 30)
+    perm = rng.permutation(777)
+    assert o.polar_energy_fixed(mu2[perm], E2[perm]) == e_fix
