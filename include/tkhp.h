@@ -75,7 +75,7 @@ enum {
 
 typedef struct {
     int32_t n_atoms;     /* N >= 1 */
-    int32_t precision;   /* TKHP_FP64 | TKHP_MIXED */
+    int32_t precision;   /* TKHP_FP64 | TKHP_MIXED | TKHP_FIXED */
     int32_t device;      /* CUDA device ordinal */
     int32_t list_mode;   /* TKHP_LIST_TILES | TKHP_LIST_CLUSTER | TKHP_LIST_ATOM */
     double box;          /* cubic box edge L; <= 0: open boundary, no images (tests) */
@@ -101,12 +101,16 @@ enum {
                                       co-resident; k_pcg_tiles: TILES mode, at most 16,384 padded atoms, any
                                       precision); the launch-per-matvec loop is used instead */
     TKHP_SOLVER_NO_FUSED_STEP = 2, /* launch-per-matvec path: update and direction as two kernels */
-    TKHP_SOLVER_STORED_T = 4       /* MIXED/FIXED precision, ATOM lists: precompute the real-space matrix elements
+    TKHP_SOLVER_STORED_T = 4,      /* MIXED/FIXED precision, ATOM lists: precompute the real-space matrix elements
                                       (two radial factors per list slot, 8 bytes) after a list build and stream
                                       them in every T.mu product instead of re-evaluating the
                                       radial functions; tkhp_tmatvec and the launch-per-matvec solve use it, the
                                       persistent solve kernel is not used.  Adds 8 bytes per list slot of capacity
                                       to the workspace. */
+    TKHP_SOLVER_TEST_BARRIER_FAULT = 8 /* tests only: the last CTA of a persistent solve kernel returns before its first
+                                      grid barrier, as a CTA lost to a fault would.  The others give up after 2 s, the
+                                      kernel leaves d_mu untouched, and tkhp_polar_solve repeats the solve on the
+                                      launch-per-matvec path (as after any barrier time-out) and keeps to that path */
 };
 
 /* Bytes of device workspace tkhp_create() needs for these parameters.  Host, pure. */
@@ -142,7 +146,11 @@ const char *tkhp_last_error(const tkhp_ctx *ctx);
  * walks all mates of an atom's group on one thread.
  * On a stream of the caller's (not the legacy default stream 0) the whole build is
  * captured once into a CUDA graph, keyed by the three input pointers, and replayed by
- * later calls with the same pointers; contents may change freely between calls.
+ * later calls with the same pointers; contents may change freely between calls.  The graphs
+ * of the four most recently used pointer triples are kept (an integrator that alternates
+ * between position buffers does not re-capture); a fifth triple replaces the least recently
+ * used one.  If `stream` is being captured by the caller, or a capture ever fails, the build
+ * is enqueued as plain launches instead; tkhp_profile_read_build() counts each case.
  */
 int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polarizability,
                       const int32_t *d_group_id, void *stream);
@@ -198,6 +206,10 @@ int tkhp_tmatvec(tkhp_ctx *ctx, const double *d_mu, double *d_out, void *stream)
  *   h_iters   host out: number of T.p products in the loop;  h_rms host out: final rms
  * Synchronises `stream` (convergence is read back by the host).  Returns TKHP_ENOCONV
  * (with the best mu) when max_iter is reached.
+ * The persistent solve kernels synchronise their CTAs with grid barriers that give up after 2 s
+ * (%globaltimer).  A solve whose barrier broke writes nothing to d_mu; the call then repeats it
+ * with one launch per product, and the context uses that path from then on
+ * (tkhp_profile_read_build out[4] counts these events).
  */
 int tkhp_polar_solve(tkhp_ctx *ctx, const double *d_field, double *d_mu, double tol,
                      int32_t max_iter, int32_t use_guess, int32_t *h_iters, double *h_rms,
@@ -283,12 +295,23 @@ int tkhp_profile_read(tkhp_ctx *ctx, int64_t *n_kernel_launches, int32_t *n_tmat
  * cooperative launch): recorded launches since the reset, their summed
  * duration in ms and the T.mu products they performed (iterations + 1 per solve). */
 int tkhp_profile_read_solve(tkhp_ctx *ctx, int32_t *n_solve_kernels, double *solve_kernel_ms, int64_t *n_matvecs);
+/* How the list builds of this context ran since tkhp_create (host counters, no synchronisation):
+ * out[0] = build graphs captured and instantiated (each costs far more host time than a replay saves:
+ * a number that grows with every build means the caller passes ever new pointers), out[1] = builds
+ * replayed from a cached graph, out[2] = builds enqueued as plain launches (legacy stream 0, caller's
+ * stream under capture, or graphs switched off), out[3] = 1 if a failed capture has switched graphs
+ * off for this context; and, kept with them although it concerns the solve, out[4] = persistent solves
+ * abandoned on a broken grid barrier and repeated on the launch-per-matvec path. */
+int tkhp_profile_read_build(tkhp_ctx *ctx, int64_t out[5]);
 
 /*
  * Register-resident FMA microbenchmark used as the measured ALU roofline denominator
  * (SURVEY 8(d) "Peaks"): runs dependent-chain FMAs with 8 accumulators per thread on every
  * SM for about `seconds`, returns sustained TFLOP/s (2 flops per FMA).
  *   precision: TKHP_MIXED -> FP32 FFMA, TKHP_FP64 -> DFMA.   Synchronises.
+ * A benchmark helper outside the "no allocation after tkhp_create()" rule: it needs no context,
+ * makes `device` current for the measurement (the caller's current device is restored on return)
+ * and allocates and frees one scalar with cudaMalloc/cudaFree and two events.
  */
 int tkhp_fma_peak(int32_t device, int32_t precision, double seconds, double *tflops);
 

@@ -12,6 +12,7 @@ TKHP_ENOCONV, TKHP_ECAPACITY, TKHP_ENONFINITE = -5, -6, -7
 TKHP_FP64, TKHP_MIXED, TKHP_FIXED = 0, 1, 2
 TKHP_LIST_TILES, TKHP_LIST_CLUSTER, TKHP_LIST_ATOM = 0, 1, 2
 TKHP_SOLVER_NO_PERSISTENT, TKHP_SOLVER_NO_FUSED_STEP, TKHP_SOLVER_STORED_T = 1, 2, 4
+TKHP_SOLVER_TEST_BARRIER_FAULT = 8
 TKHP_STATIC_MAX_ATOMS = 4194304
 
 _ERR_NAMES = {-1: "TKHP_EINVAL", -2: "TKHP_ECUDA", -3: "TKHP_ECUTOFF", -4: "TKHP_ENOLIST",
@@ -22,7 +23,7 @@ EXPORTED_SYMBOLS = [
     "tkhp_nblist_build", "tkhp_nblist_view", "tkhp_nblist_stats", "tkhp_nblist_atom_stats", "tkhp_perm_field",
     "tkhp_tmatvec", "tkhp_polar_solve", "tkhp_polar_energy", "tkhp_polar_energy_static", "tkhp_polarize_host",
     "tkhp_last_timings", "tkhp_fma_peak", "tkhp_profile_reset", "tkhp_profile_read",
-    "tkhp_profile_read_solve",
+    "tkhp_profile_read_solve", "tkhp_profile_read_build",
 ]
 
 
@@ -85,6 +86,7 @@ def lib() -> ctypes.CDLL:
         L.tkhp_profile_read.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int32),
                                         POINTER(c_double), POINTER(c_int32), POINTER(c_double)]
         L.tkhp_profile_read_solve.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_double), POINTER(c_int64)]
+        L.tkhp_profile_read_build.argtypes = [c_void_p, POINTER(c_int64)]
         for name in EXPORTED_SYMBOLS:
             if name != "tkhp_last_error":
                 getattr(L, name).restype = ctypes.c_int
@@ -253,6 +255,15 @@ def tkhp_profile_read_solve(ctx):
     return dict(n_solve=n.value, solve_ms=ms.value, solve_matvecs=mv.value)
 
 
+def tkhp_profile_read_build(ctx):
+    """-> dict(graph_captures, graph_replays, plain_builds, graphs_off) of this context's list builds,
+    plus barrier_timeouts (persistent solves repeated on the launch-per-matvec path)."""
+    out = (c_int64 * 5)()
+    _check(lib().tkhp_profile_read_build(ctx, out), ctx)
+    return dict(graph_captures=int(out[0]), graph_replays=int(out[1]), plain_builds=int(out[2]),
+                graphs_off=bool(out[3]), barrier_timeouts=int(out[4]))
+
+
 def tkhp_fma_peak(device: int, precision: int, seconds: float = 2.0) -> float:
     out = c_double(0.0)
     _check(lib().tkhp_fma_peak(device, precision, seconds, byref(out)))
@@ -367,7 +378,7 @@ class Polarizer:
     def polar_energy(self, mu, field, stream=None):
         """-> 0-d CUDA float64 tensor (kcal/mol)."""
         out = self.torch.empty((), dtype=self.torch.float64, device=self.device)
-        tkhp_polar_energy(self.ctx, self._f64(mu), self._f64(field), out, stream)
+        tkhp_polar_energy(self.ctx, self._f64(mu), self._f64(field), out, self._s(stream))
         return out
 
     def timings(self):

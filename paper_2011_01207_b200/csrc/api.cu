@@ -37,7 +37,7 @@ static int check_params(const tkhp_params *p, char *err, size_t n) {
     }
     if (p->precision != TKHP_FP64 && p->n_atoms > (1 << 24)) { snprintf(err, n, "MIXED / FIXED precision supports up to 2^24 atoms"); return TKHP_EINVAL; }
     if (p->max_tiles_per_block < 0 || p->max_nbrs_per_cluster < 0 || p->max_nbrs_per_atom < 0) { snprintf(err, n, "negative capacity"); return TKHP_EINVAL; }
-    if (p->solver_flags & ~(TKHP_SOLVER_NO_PERSISTENT | TKHP_SOLVER_NO_FUSED_STEP | TKHP_SOLVER_STORED_T) || p->reserved != 0) { snprintf(err, n, "unknown solver_flags / non-zero reserved field"); return TKHP_EINVAL; }
+    if (p->solver_flags & ~(TKHP_SOLVER_NO_PERSISTENT | TKHP_SOLVER_NO_FUSED_STEP | TKHP_SOLVER_STORED_T | TKHP_SOLVER_TEST_BARRIER_FAULT) || p->reserved != 0) { snprintf(err, n, "unknown solver_flags / non-zero reserved field"); return TKHP_EINVAL; }
     if (p->max_stage_per_chunk < 0 || (p->max_stage_per_chunk & 31)) { snprintf(err, n, "max_stage_per_chunk must be a non-negative multiple of 32"); return TKHP_EINVAL; }
     return TKHP_OK;
 }
@@ -181,6 +181,28 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
+// Destroys whatever a (possibly half-built: zero-filled at birth) context owns besides the caller's workspace.
+// The context's device is current.
+static void release_ctx(Ctx *c) {
+    for (int i = 0; i < 10; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < 2; ++i) if (c->copy_ev[i]) cudaEventDestroy(c->copy_ev[i]);
+    for (int i = 0; i < 2; ++i) {
+        if (c->side[i]) cudaStreamDestroy(c->side[i]);
+        if (c->fork_ev[i]) cudaEventDestroy(c->fork_ev[i]);
+        if (c->join_ev[i]) cudaEventDestroy(c->join_ev[i]);
+    }
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    for (int w = 0; w < 3; ++w)
+        for (int i = 0; i < 2 * PROF_MAX; ++i) if (c->prof_ev[w][i]) cudaEventDestroy(c->prof_ev[w][i]);
+    for (int i = 0; i < Ctx::BUILD_GRAPH_SLOTS; ++i)
+        if (c->build_slot[i].exec) cudaGraphExecDestroy(c->build_slot[i].exec);
+    if (c->h_ring) cudaFreeHost(c->h_ring);
+    if (c->h_scalars) cudaFreeHost(c->h_scalars);
+    if (c->h_state) cudaFreeHost(c->h_state);
+    cudaGetLastError();
+    delete c;
+}
+
 extern "C" {
 
 int tkhp_workspace_bytes(const tkhp_params *params, size_t *bytes) {
@@ -205,30 +227,37 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
         cudaGetLastError();
         return TKHP_ECUDA;
     }
-    int prev_device = -1;
-    cudaGetDevice(&prev_device);
-    if (cudaSetDevice(params->device) != cudaSuccess) { snprintf(g_create_err, sizeof(g_create_err), "cudaSetDevice failed"); return TKHP_ECUDA; }
+    DeviceGuard guard(params->device);      // the caller's current device comes back on every return path
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != params->device) { snprintf(g_create_err, sizeof(g_create_err), "cudaSetDevice failed"); cudaGetLastError(); return TKHP_ECUDA; }
     Ctx *c = new (std::nothrow) Ctx();
-    if (!c) return TKHP_EINVAL;
+    if (!c) { snprintf(g_create_err, sizeof(g_create_err), "out of host memory"); return TKHP_EINVAL; }
     memset(c, 0, sizeof(Ctx));
     c->p = *params;
+    // every failure below leaves through here: whatever was created so far is destroyed again
+    auto fail = [&](int code, const char *msg) {
+        snprintf(g_create_err, sizeof(g_create_err), "%s", msg);
+        release_ctx(c);
+        return code;
+    };
     size_t need = carve(c, params, d_workspace);
     if (bytes < need) {
-        snprintf(g_create_err, sizeof(g_create_err), "workspace too small: %zu < %zu bytes", bytes, need);
-        delete c;
-        return TKHP_ECAPACITY;
+        char msg[128];
+        snprintf(msg, sizeof(msg), "workspace too small: %zu < %zu bytes", bytes, need);
+        return fail(TKHP_ECAPACITY, msg);
     }
     cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, params->device) != cudaSuccess) { delete c; return TKHP_ECUDA; }
+    if (cudaGetDeviceProperties(&prop, params->device) != cudaSuccess) return fail(TKHP_ECUDA, "cudaGetDeviceProperties failed");
     c->sm_count = prop.multiProcessorCount;
     atom_far_setup(c);
     c->fixed = params->precision == TKHP_FIXED;
     c->no_persist = (params->solver_flags & TKHP_SOLVER_NO_PERSISTENT) != 0;
     c->no_fused_step = (params->solver_flags & TKHP_SOLVER_NO_FUSED_STEP) != 0;
+    c->test_barrier_fault = (params->solver_flags & TKHP_SOLVER_TEST_BARRIER_FAULT) != 0;
     if (cluster_pairs_configure(c) || atom_lists_configure(c) || atom_pairs_configure(c) || atom_solve_configure(c) || atom_stored_configure(c)) {
-        snprintf(g_create_err, sizeof(g_create_err), "%s", c->err);
-        delete c;
-        return TKHP_ECUDA;
+        char msg[sizeof(c->err)];
+        snprintf(msg, sizeof(msg), "%s", c->err);
+        return fail(TKHP_ECUDA, msg);
     }
     c->spec_iter = -1;
     c->fuse_q = false;
@@ -237,29 +266,28 @@ int tkhp_create(const tkhp_params *params, void *d_workspace, size_t bytes, tkhp
     if (cudaHostAlloc(&c->h_ring, RING * sizeof(double), cudaHostAllocMapped) != cudaSuccess ||
         cudaHostGetDevicePointer(&c->d_ring, c->h_ring, 0) != cudaSuccess ||
         cudaMallocHost(&c->h_scalars, 8 * sizeof(double)) != cudaSuccess ||
-        cudaMallocHost(&c->h_state, sizeof(DeviceState)) != cudaSuccess) {
-        snprintf(g_create_err, sizeof(g_create_err), "cudaMallocHost failed");
-        delete c;
-        return TKHP_ECUDA;
-    }
-    for (int i = 0; i < 10; ++i) cudaEventCreate(&c->ev[i]);
-    cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
-    for (int i = 0; i < 2; ++i) cudaEventCreateWithFlags(&c->copy_ev[i], cudaEventDisableTiming);
+        cudaMallocHost(&c->h_state, sizeof(DeviceState)) != cudaSuccess)
+        return fail(TKHP_ECUDA, "cudaMallocHost failed");
+    bool ok = true;
+    for (int i = 0; i < 10; ++i) ok &= cudaEventCreate(&c->ev[i]) == cudaSuccess;
+    ok &= cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+    for (int i = 0; i < 2; ++i) ok &= cudaEventCreateWithFlags(&c->copy_ev[i], cudaEventDisableTiming) == cudaSuccess;
     for (int i = 0; i < 2; ++i) {
-        cudaStreamCreateWithFlags(&c->side[i], cudaStreamNonBlocking);
-        cudaEventCreateWithFlags(&c->fork_ev[i], cudaEventDisableTiming);
-        cudaEventCreateWithFlags(&c->join_ev[i], cudaEventDisableTiming);
+        ok &= cudaStreamCreateWithFlags(&c->side[i], cudaStreamNonBlocking) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&c->fork_ev[i], cudaEventDisableTiming) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&c->join_ev[i], cudaEventDisableTiming) == cudaSuccess;
     }
     for (int w = 0; w < 3; ++w)
-        for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventCreate(&c->prof_ev[w][i]);
+        for (int i = 0; i < 2 * PROF_MAX; ++i) ok &= cudaEventCreate(&c->prof_ev[w][i]) == cudaSuccess;
+    if (!ok) return fail(TKHP_ECUDA, "creating the context's streams and events failed");
     for (int i = 0; i < 5; ++i) c->last_ms[i] = -1.0;
     c->built = false;
     c->tstore_valid = false;
     c->header_valid = false;
     c->list_mode_in_use = TKHP_LIST_TILES;
     // the device-resident scalars start from zero (tickets, barrier words: tkhp_polar_energy may be the first call)
-    if (cudaMemset(c->st, 0, sizeof(DeviceState)) != cudaSuccess || cluster_init(c) != TKHP_OK || cudaDeviceSynchronize() != cudaSuccess) { delete c; return TKHP_ECUDA; }
-    if (prev_device >= 0 && prev_device != params->device) cudaSetDevice(prev_device);      // leave the caller's current device as it was
+    if (cudaMemset(c->st, 0, sizeof(DeviceState)) != cudaSuccess || cluster_init(c) != TKHP_OK || cudaDeviceSynchronize() != cudaSuccess)
+        return fail(TKHP_ECUDA, "initialising the workspace failed");
     *out = reinterpret_cast<tkhp_ctx *>(c);
     return TKHP_OK;
 }
@@ -269,17 +297,7 @@ int tkhp_destroy(tkhp_ctx *ctx) {
     Ctx *c = reinterpret_cast<Ctx *>(ctx);
     DeviceGuard guard(c->p.device);
     cudaDeviceSynchronize();
-    for (int i = 0; i < 10; ++i) cudaEventDestroy(c->ev[i]);
-    for (int i = 0; i < 2; ++i) cudaEventDestroy(c->copy_ev[i]);
-    for (int i = 0; i < 2; ++i) { cudaStreamDestroy(c->side[i]); cudaEventDestroy(c->fork_ev[i]); cudaEventDestroy(c->join_ev[i]); }
-    cudaStreamDestroy(c->copy_stream);
-    for (int w = 0; w < 3; ++w)
-        for (int i = 0; i < 2 * PROF_MAX; ++i) cudaEventDestroy(c->prof_ev[w][i]);
-    if (c->build_graph) cudaGraphExecDestroy(c->build_graph);
-    cudaFreeHost(c->h_ring);
-    cudaFreeHost(c->h_scalars);
-    cudaFreeHost(c->h_state);
-    delete c;
+    release_ctx(c);
     return TKHP_OK;
 }
 
@@ -310,22 +328,39 @@ int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polari
     tic(c, 0, s);
     c->header_valid = false;
     int rc = TKHP_OK;
-    const bool same = c->build_graph && c->build_key[0] == d_pos && c->build_key[1] == d_polarizability &&
-                      c->build_key[2] == d_group_id;
-    if (!same && !c->no_graph && s != nullptr) {
-        // capture the build once for these pointers (the legacy default stream cannot be captured)
-        if (c->build_graph) { cudaGraphExecDestroy(c->build_graph); c->build_graph = nullptr; }
+    auto find_slot = [&]() {
+        for (int i = 0; i < Ctx::BUILD_GRAPH_SLOTS; ++i) {
+            const Ctx::BuildGraphSlot &g = c->build_slot[i];
+            if (g.exec && g.key[0] == d_pos && g.key[1] == d_polarizability && g.key[2] == d_group_id) return i;
+        }
+        return -1;
+    };
+    // a caller who is capturing `s` into a graph of their own gets plain launches (they become nodes of that
+    // graph); beginning a second capture on the stream would fail and replaying ours would nest it
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    const bool caller_capturing = s != nullptr && (cudaStreamIsCapturing(s, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone);
+    int slot = find_slot();
+    if (slot < 0 && !c->no_graph && s != nullptr && !caller_capturing) {
+        // capture the build once for these pointers (the legacy default stream cannot be captured) into the
+        // least recently used slot
+        int victim = 0;
+        for (int i = 1; i < Ctx::BUILD_GRAPH_SLOTS; ++i)
+            if (c->build_slot[i].used < c->build_slot[victim].used) victim = i;
+        Ctx::BuildGraphSlot &g = c->build_slot[victim];
+        if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+        g.used = 0;
         cudaGraph_t graph = nullptr;
         const long long before = c->n_launches;
         if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
             rc = enqueue_build(c, d_pos, d_polarizability, d_group_id, s);
             const cudaError_t e = cudaStreamEndCapture(s, &graph);
-            if (rc == TKHP_OK && e == cudaSuccess && graph &&
-                cudaGraphInstantiate(&c->build_graph, graph, 0) == cudaSuccess) {
-                c->build_key[0] = d_pos; c->build_key[1] = d_polarizability; c->build_key[2] = d_group_id;
-                c->build_graph_launches = c->n_launches - before;
+            if (rc == TKHP_OK && e == cudaSuccess && graph && cudaGraphInstantiate(&g.exec, graph, 0) == cudaSuccess) {
+                g.key[0] = d_pos; g.key[1] = d_polarizability; g.key[2] = d_group_id;
+                g.launches = c->n_launches - before;
+                c->n_graph_captures += 1;
+                slot = victim;
             } else {
-                c->build_graph = nullptr;
+                g.exec = nullptr;
                 c->no_graph = true;
                 rc = TKHP_OK;
             }
@@ -336,12 +371,15 @@ int tkhp_nblist_build(tkhp_ctx *ctx, const double *d_pos, const double *d_polari
         }
         cudaGetLastError();
     }
-    if (c->build_graph && c->build_key[0] == d_pos && c->build_key[1] == d_polarizability && c->build_key[2] == d_group_id) {
-        TKHP_CUDA(c, cudaGraphLaunch(c->build_graph, s));
-        c->n_launches += c->build_graph_launches;
+    if (slot >= 0 && !caller_capturing) {
+        TKHP_CUDA(c, cudaGraphLaunch(c->build_slot[slot].exec, s));
+        c->build_slot[slot].used = ++c->build_clock;
+        c->n_launches += c->build_slot[slot].launches;
+        c->n_graph_replays += 1;
     } else {
         rc = enqueue_build(c, d_pos, d_polarizability, d_group_id, s);
         if (rc) return rc;
+        c->n_plain_builds += 1;
     }
     c->built = true;
     c->tstore_valid = false;               // stored matrix elements belong to the previous list
@@ -562,6 +600,17 @@ int tkhp_profile_read_solve(tkhp_ctx *ctx, int32_t *n_solve_kernels, double *sol
     if (n_solve_kernels) *n_solve_kernels = c->prof_n[2];
     if (solve_kernel_ms) *solve_kernel_ms = tot;
     if (n_matvecs) *n_matvecs = c->prof_solve_matvecs;
+    return TKHP_OK;
+}
+
+int tkhp_profile_read_build(tkhp_ctx *ctx, int64_t out[5]) {
+    if (!ctx || !out) return TKHP_EINVAL;
+    const Ctx *c = reinterpret_cast<const Ctx *>(ctx);
+    out[0] = c->n_graph_captures;
+    out[1] = c->n_graph_replays;
+    out[2] = c->n_plain_builds;
+    out[3] = c->no_graph ? 1 : 0;
+    out[4] = c->n_barrier_timeouts;
     return TKHP_OK;
 }
 

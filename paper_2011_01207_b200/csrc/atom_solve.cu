@@ -46,6 +46,7 @@ struct SolveArgs {
     DeviceState *st;
     double tol, self;
     int max_iter, n_atoms, n_pad, s_chunk, rot_div;
+    int test_fault;          // TKHP_SOLVER_TEST_BARRIER_FAULT: the last CTA never arrives at the first barrier
 };
 
 __host__ __device__ inline size_t solve_smem(int s_chunk, bool split) {
@@ -138,13 +139,14 @@ k_pcg_persist(SolveArgs a) {
         a.mu0[slot] = make_float4((float)m0[0], (float)m0[1], (float)m0[2], 0.f);
     }
     unsigned gen = 0;
-    grid_barrier(st, gen);
+    if (a.test_fault && g == (int)gridDim.x - 1) return;      // tests: a CTA that is lost before the first barrier
+    bool broken = !grid_barrier(st, gen);        // a barrier timed out: leave without touching the caller's mu
     double rz_old = 0.0, rr = 0.0;
     float delta = 0.f;
     int it = 0;                                  // iterations completed
     bool converged = false;
 
-    for (int k = -1; k < a.max_iter; ++k) {
+    for (int k = -1; k < a.max_iter && !broken; ++k) {
         // ---- operand: p_j <- u_j + delta p_j for every staged atom (k = -1: mu0; k = 0: delta = 0)
         __syncthreads();
         for (int l = t; l < count; l += GT) {
@@ -201,7 +203,7 @@ k_pcg_persist(SolveArgs a) {
             }
             block_sum2(s1, s2);
             if (t == 0) { a.part_a[2 * g] = s1; a.part_a[2 * g + 1] = s2; }
-            grid_barrier(st, gen);
+            if (!grid_barrier(st, gen)) { broken = true; break; }
             grid_totals(a.part_a, rz_old, rr);
             delta = 0.f;
             if (sqrt(rr / a.n_atoms) < a.tol) { converged = true; break; }
@@ -219,7 +221,7 @@ k_pcg_persist(SolveArgs a) {
         }
         block_sum2(s1, s2);
         if (t == 0) { a.part_b[2 * g] = s1; a.part_b[2 * g + 1] = 0.0; }
-        grid_barrier(st, gen);
+        if (!grid_barrier(st, gen)) { broken = true; break; }
         double pq, unused;
         grid_totals(a.part_b, pq, unused);
         const double gamma = rz_old / pq;
@@ -240,7 +242,7 @@ k_pcg_persist(SolveArgs a) {
         }
         block_sum2(s1, s2);
         if (t == 0) { a.part_a[2 * g] = s1; a.part_a[2 * g + 1] = s2; }
-        grid_barrier(st, gen);
+        if (!grid_barrier(st, gen)) { broken = true; break; }
         double rz_new;
         grid_totals(a.part_a, rz_new, rr);
         it = k + 1;
@@ -253,7 +255,7 @@ k_pcg_persist(SolveArgs a) {
         }
     }
     // ---- result, in the caller's order; the scalars go to host-mapped memory
-    if (owner && atom >= 0) {
+    if (owner && atom >= 0 && !broken) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) a.mu[3 * (size_t)atom + c] = s_vec[c * GT + t];
     }
@@ -263,7 +265,7 @@ k_pcg_persist(SolveArgs a) {
         st->conv_at = converged ? it : 0x7fffffff;
         a.result[0] = rr;
         a.result[1] = (double)it;
-        a.result[2] = (double)st->err_barrier;
+        a.result[2] = broken ? 1.0 : 0.0;        // CTA 0 learns of a broken barrier no later than at its own next one
         __threadfence_system();
     }
 }
@@ -342,6 +344,7 @@ int atom_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_guess
     a.n_pad = c->n_pad;
     a.s_chunk = (c->h_state->max_stage + 31) & ~31;
     a.rot_div = c->sm_count;
+    a.test_fault = c->test_barrier_fault ? 1 : 0;
     TKHP_CUDA(c, cudaMemsetAsync(&c->st->bar_count, 0, 2 * sizeof(unsigned), s));
     void *args[] = {&a};
     if (cudaLaunchCooperativeKernel(pick(c, ws), dim3(ws.n_groups), dim3(GT), args, solve_smem(a.s_chunk, c->n_blocks / ws.n_groups < 5), s) != cudaSuccess)

@@ -26,7 +26,8 @@ struct DeviceState {
     int err_bad_alpha;      // alpha <= 0
     int err_bad_group;      // group id outside [0, N)
     int err_capacity;       // tile list or cluster list overflow
-    int err_barrier;        // a grid barrier of the persistent PCG kernel timed out
+    int err_barrier;        // a grid barrier of a persistent PCG kernel timed out (diagnostic, sticky until the next build;
+                            // the kernels report a broken barrier through their result slot, not through this flag)
     int pad_err;
     // grid (sort key)
     int grid_bits;          // b
@@ -127,6 +128,8 @@ struct Ctx {
     bool fixed;             // TKHP_FIXED: int64 fixed-point accumulators in the FP32 pair kernels and the energy
     bool coop_ok;           // the device supports cooperative launches
     bool no_persist, no_fused_step;   // tkhp_params.solver_flags
+    bool test_barrier_fault;          // TKHP_SOLVER_TEST_BARRIER_FAULT (tests: one CTA of the persistent kernels is lost)
+    long long n_barrier_timeouts;     // persistent solves given up on a broken grid barrier and repeated on the fall-back path
     bool fuse_q;            // ATOM-mode T.mu kernel also forms q = p/alpha - T p - self p and p.q (PCG)
     int spec_iter;          // >= 0: the pair kernel about to be launched belongs to PCG iteration spec_iter
     DeviceState *h_state;   // pinned host copy of *st (list header), valid when header_valid
@@ -145,12 +148,22 @@ struct Ctx {
     void *cl_ws;
     size_t cl_ws_bytes;
 
-    // CUDA graph of one whole list build (about 30 small kernels, memsets and copies: launch bound),
-    // re-used while the caller passes the same input pointers
-    cudaGraphExec_t build_graph;
-    const void *build_key[3];           // d_pos, d_polarizability, d_group_id the graph was captured with
-    long long build_graph_launches;     // kernels inside the graph
+    // CUDA graphs of one whole list build (about 30 small kernels, memsets and copies: launch bound).
+    // A graph holds the three input pointers it was captured with; an MD integrator usually alternates
+    // between two or three position buffers, so the last BUILD_GRAPH_SLOTS pointer triples keep their
+    // graphs (least recently used slot is re-captured).
+    static constexpr int BUILD_GRAPH_SLOTS = 4;
+    struct BuildGraphSlot {
+        cudaGraphExec_t exec;
+        const void *key[3];             // d_pos, d_polarizability, d_group_id the graph was captured with
+        long long launches;             // kernels inside the graph
+        unsigned long long used;        // value of build_clock at the last replay (0: never)
+    } build_slot[BUILD_GRAPH_SLOTS];
+    unsigned long long build_clock;
     bool no_graph;                      // capture failed once: plain launches from then on
+    long long n_graph_captures;         // graphs captured and instantiated since tkhp_create
+    long long n_graph_replays;          // builds that ran as a graph replay
+    long long n_plain_builds;           // builds enqueued as plain launches (stream 0, caller capturing, no_graph)
 
     cudaEvent_t ev[10];
     double last_ms[5];

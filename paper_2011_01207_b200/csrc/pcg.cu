@@ -317,16 +317,22 @@ k_energy(const double *__restrict__ mu, const double *__restrict__ field, long l
     if (grid_sum2_last_block(part, &st->ticket, s, dmy) && threadIdx.x == 0) *energy = -0.5 * COULOMB * s;
 }
 
-// TKHP_FIXED: every term -1/2 f mu_i.E_i goes into an int64 container with 30 fractional
-// bits (kcal/mol); integer sums do not depend on the order, so warp sums and one integer atomic per
-// warp are deterministic.  The last block converts back (eq. 3) and clears the container.
+// TKHP_FIXED (Q21): every ATOM's term -1/2 f mu_i.E_i goes into an int64 container
+// with 30 fractional bits (kcal/mol) -- one conversion per atom, of the dot product ((x + y) + z) formed
+// without fused multiply-adds, so that the integer is a defined function of the inputs.  Integer sums do not
+// depend on the order, so warp sums and one integer atomic per warp are deterministic.  The last block
+// converts back (eq. 3) and clears the container.  __double2ll_rn saturates: a term of 2^33 kcal/mol or more
+// cannot be held (the paper's mode has no guard against that either).
 __global__ void __launch_bounds__(RED_THREADS)
-k_energy_fixed(const double *__restrict__ mu, const double *__restrict__ field, long long n3, DeviceState *st,
+k_energy_fixed(const double *__restrict__ mu, const double *__restrict__ field, long long n_atoms, DeviceState *st,
                double *__restrict__ energy) {
     long long s = 0;
     const double scale = -0.5 * COULOMB * (double)(1ll << FIX_ENERGY_BITS);
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += (long long)gridDim.x * blockDim.x)
-        s += __double2ll_rn(mu[i] * field[i] * scale);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_atoms; i += (long long)gridDim.x * blockDim.x) {
+        const double *m = mu + 3 * i, *e = field + 3 * i;
+        const double dot = __dadd_rn(__dadd_rn(__dmul_rn(m[0], e[0]), __dmul_rn(m[1], e[1])), __dmul_rn(m[2], e[2]));
+        s += __double2ll_rn(__dmul_rn(dot, scale));
+    }
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if ((threadIdx.x & 31) == 0) atomicAdd(&st->energy_fixed, (unsigned long long)s);
     __shared__ bool s_last;
@@ -487,7 +493,15 @@ int do_polar_solve(Ctx *c, const double *d_field, double *d_mu, double tol, int 
         TKHP_CUDA(c, e);
         const int it_done = (int)c->h_ring[1];
         const double rms_done = sqrt(c->h_ring[0] / c->n);
-        if (c->h_ring[2] != 0.0) return set_err(c, TKHP_ECUDA, "grid barrier of the persistent PCG kernel timed out%s");
+        if (c->h_ring[2] != 0.0) {
+            // A grid barrier of the persistent kernel timed out (a CTA never arrived within 2 s).  The kernel left
+            // d_mu as the caller passed it, so nothing is lost: this context stops using persistent kernels and the
+            // solve is repeated on the launch-per-matvec path.
+            c->no_persist = true;
+            c->n_barrier_timeouts += 1;
+            if (rec) c->prof_n[2]--;
+            return do_polar_solve(c, d_field, d_mu, tol, max_iter, use_guess, h_iters, h_rms, s);
+        }
         if (rec) c->prof_solve_matvecs += it_done + 1;
         if (h_iters) *h_iters = it_done;
         if (h_rms) *h_rms = rms_done;
@@ -581,7 +595,7 @@ int do_polar_energy(Ctx *c, const double *d_mu, const double *d_field, double *d
     int g = div_up(n3, VEC_THREADS);
     if (g > MAX_PARTIALS) g = MAX_PARTIALS;
     double *part = c->partials + 4 * (size_t)c->part_cap;
-    if (c->fixed) k_energy_fixed<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, c->st, d_energy);
+    if (c->fixed) k_energy_fixed<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, (long long)c->n, c->st, d_energy);
     else k_energy<<<g, VEC_THREADS, 0, s>>>(d_mu, d_field, n3, part, c->st, d_energy);
     c->n_launches += 1;
     TKHP_CUDA(c, cudaGetLastError());

@@ -74,23 +74,47 @@ __device__ __forceinline__ unsigned ld_acquire(const unsigned *p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+constexpr unsigned BAR_POISON = 0x80000000u;                 // bit 31 of bar_count: some CTA gave up waiting
+constexpr unsigned long long BAR_TIMEOUT_NS = 2000000000ull; // 2 s of %globaltimer, whatever the clocks are
+
 // All threads of all CTAs.  `gen` counts the barriers this CTA has passed.  One atomic per CTA on a
 // counter that only grows during a solve; everybody spins on the counter itself (one L2 round trip
 // less on the critical path than a separate release word written by the last arriver).
-__device__ __forceinline__ void grid_barrier(DeviceState *st, unsigned &gen) {
+// Returns false (uniformly over the CTA) when the barrier is broken: a CTA that has waited for
+// BAR_TIMEOUT_NS sets bit 31 of the counter, which every other CTA sees in the value it polls or in
+// the value its own arrival returns -- at this barrier or at its next one, with no extra memory
+// access on the good path.  After `false` the partial sums are inconsistent: the caller must leave
+// its loop without writing results.  (The arrival counts stay far below 2^31: barriers per solve x CTAs.)
+__device__ __forceinline__ bool grid_barrier(DeviceState *st, unsigned &gen) {
+    int bad = 0;
     __syncthreads();
     ++gen;
     if (threadIdx.x == 0) {
         __threadfence();
         const unsigned target = gen * gridDim.x;
-        if (atomicAdd(&st->bar_count, 1u) + 1u != target) {
-            // bounded spin (a few seconds): a CTA that never arrives must not hang the device
-            for (unsigned n = 0; ld_acquire(&st->bar_count) < target; ++n)
-                if (n > (1u << 22)) { st->err_barrier = 1; break; }
+        unsigned v = atomicAdd(&st->bar_count, 1u) + 1u;
+        if (v < target) {
+            unsigned long long t0 = 0;
+            for (unsigned n = 1; (v = ld_acquire(&st->bar_count)) < target; ++n) {
+                if ((n & 0x3ffu) != 0) continue;                      // look at the clock every 1024 polls
+                const unsigned long long now = global_ns();
+                if (t0 == 0) t0 = now;
+                else if (now - t0 > BAR_TIMEOUT_NS) {
+                    v = atomicOr(&st->bar_count, BAR_POISON) | BAR_POISON;
+                    st->err_barrier = 1;
+                    break;
+                }
+            }
         }
+        bad = (v & BAR_POISON) != 0u;
         __threadfence();
     }
-    __syncthreads();
+    return __syncthreads_or(bad) == 0;      // the closing CTA barrier also hands thread 0's verdict to everybody
 }
 
 // identical in every CTA: sum of the per-CTA partials in a fixed order

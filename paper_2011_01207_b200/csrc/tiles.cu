@@ -253,6 +253,7 @@ struct TilesSolveArgs {
     double box, tol, self;
     long long n_tiles;
     int n_pad, n_atoms, max_iter, use_guess;
+    int test_fault;            // TKHP_SOLVER_TEST_BARRIER_FAULT: the last CTA never arrives at the first barrier
 };
 
 template <typename real, bool PPI>
@@ -288,15 +289,16 @@ k_pcg_tiles(TilesSolveArgs a, PairConsts<real> kc) {
         mu[s] = v;
     }
     unsigned gen = 0;
-    grid_barrier(st, gen);
+    if (a.test_fault && blockIdx.x == gridDim.x - 1) return;   // tests: a CTA that is lost before the first barrier
+    bool broken = !grid_barrier(st, gen);       // a barrier timed out: leave without touching the caller's mu
     double rz_old = 0.0, rr = 0.0;
     int it = 0;
     bool converged = false;
-    for (int k = -1; k < a.max_iter; ++k) {
+    for (int k = -1; k < a.max_iter && !broken; ++k) {
         // ---- acc = T v (v = mu0 or the direction)
         for (long long t = (long long)blockIdx.x * TILE_WARPS + w; t < a.n_tiles; t += wstride)
             tile_tmu_one<real, PPI>(a.pairs[t], s_pos, s_mu, xyzw, mu, a.bcentre, a.box, kc, a.acc, n_pad, fixed);
-        grid_barrier(st, gen);
+        if (!grid_barrier(st, gen)) { broken = true; break; }
         double s1 = 0.0, s2 = 0.0;
         if (k < 0) {
             // r = E - (mu/alpha - T mu - self mu); z = alpha r; p = z
@@ -318,7 +320,7 @@ k_pcg_tiles(TilesSolveArgs a, PairConsts<real> kc) {
             }
             block_sum2(s1, s2);
             if (threadIdx.x == 0) { part_a[2 * blockIdx.x] = s1; part_a[2 * blockIdx.x + 1] = s2; }
-            grid_barrier(st, gen);
+            if (!grid_barrier(st, gen)) { broken = true; break; }
             grid_totals(part_a, rz_old, rr);
             if (sqrt(rr / a.n_atoms) < a.tol) { converged = true; break; }
             continue;
@@ -338,7 +340,7 @@ k_pcg_tiles(TilesSolveArgs a, PairConsts<real> kc) {
         }
         block_sum2(s1, s2);
         if (threadIdx.x == 0) { part_b[2 * blockIdx.x] = s1; part_b[2 * blockIdx.x + 1] = 0.0; }
-        grid_barrier(st, gen);
+        if (!grid_barrier(st, gen)) { broken = true; break; }
         double pq, unused;
         grid_totals(part_b, pq, unused);
         const double gamma = rz_old / pq;
@@ -357,7 +359,7 @@ k_pcg_tiles(TilesSolveArgs a, PairConsts<real> kc) {
         }
         block_sum2(s1, s2);
         if (threadIdx.x == 0) { part_a[2 * blockIdx.x] = s1; part_a[2 * blockIdx.x + 1] = s2; }
-        grid_barrier(st, gen);
+        if (!grid_barrier(st, gen)) { broken = true; break; }
         double rz_new;
         grid_totals(part_a, rz_new, rr);
         it = k + 1;
@@ -377,10 +379,10 @@ k_pcg_tiles(TilesSolveArgs a, PairConsts<real> kc) {
             vec4 v; v.x = (real)p[0]; v.y = (real)p[1]; v.z = (real)p[2]; v.w = 0;
             mu[s] = v;
         }
-        grid_barrier(st, gen);
+        if (!grid_barrier(st, gen)) { broken = true; break; }
     }
     // ---- result in the caller's order; scalars to host-mapped memory
-    for (int s = tid; s < n_pad; s += nthr) {
+    for (int s = tid; s < n_pad && !broken; s += nthr) {
         const int at = a.perm[s];
         if (at >= 0) {
 #pragma unroll
@@ -393,7 +395,7 @@ k_pcg_tiles(TilesSolveArgs a, PairConsts<real> kc) {
         st->conv_at = converged ? it : 0x7fffffff;
         a.result[0] = rr;
         a.result[1] = (double)it;
-        a.result[2] = (double)st->err_barrier;
+        a.result[2] = broken ? 1.0 : 0.0;
         __threadfence_system();
     }
 }
@@ -521,6 +523,7 @@ int tiles_solve_launch(Ctx *c, const double *d_field, double *d_mu, int use_gues
     a.self = 4.0 * p.ewald_beta * p.ewald_beta * p.ewald_beta / (3.0 * SQRT_PI);
     a.n_tiles = c->h_state->n_tiles;
     a.n_pad = c->n_pad; a.n_atoms = c->n; a.max_iter = max_iter; a.use_guess = use_guess;
+    a.test_fault = c->test_barrier_fault ? 1 : 0;
     const int grid = tiles_solve_grid(c);
     TKHP_CUDA(c, cudaMemsetAsync(&c->st->bar_count, 0, 2 * sizeof(unsigned), s));
     cudaError_t e;

@@ -348,6 +348,47 @@ def test_every_solver_path_agrees_with_the_oracle(flags):
     P.close()
 
 
+@pytest.mark.parametrize("kernel", ["k_pcg_persist", "k_pcg_tiles"])
+def test_broken_grid_barrier_falls_back_to_launch_per_matvec(kernel):
+    """A persistent solve kernel whose grid barrier breaks (here: TKHP_SOLVER_TEST_BARRIER_FAULT makes
+    the last CTA leave before its first arrival; the others give up after 2 s of %globaltimer) writes
+    nothing to d_mu.  tkhp_polar_solve then repeats the solve with one launch per product:
+    same answer and iteration count as a context that never used the persistent kernel, the guess is
+    honoured, the event is counted once, and later solves stay on the fall-back path (no second wait)."""
+    import time
+    import torch
+    pk = _pk()
+    s, mode = (SYSTEMS["water_6000"](), pk.TKHP_LIST_ATOM) if kernel == "k_pcg_persist" else (SYSTEMS["cfg0"](), pk.TKHP_LIST_TILES)
+    P = pk.Polarizer.for_system(s, precision=pk.TKHP_MIXED, list_mode=mode, solver_flags=pk.TKHP_SOLVER_TEST_BARRIER_FAULT)
+    Q = pk.Polarizer.for_system(s, precision=pk.TKHP_MIXED, list_mode=mode, solver_flags=pk.TKHP_SOLVER_NO_PERSISTENT)
+    for X in (P, Q):
+        X.nblist_build(s.pos, s.polarizability, s.group_id)
+    assert P.nblist_stats(count_pairs=False)[2] == mode
+    Eg = Q.perm_field(s.charge, s.dipole, s.quad)
+    mu_q, it_q, rms_q = Q.polar_solve(Eg, tol=1e-7)
+    # a guess that is nowhere near alpha E: were it overwritten or ignored, the iteration count would differ
+    guess = mu_q * 0.5
+    mu_qg, it_qg, _ = Q.polar_solve(Eg, tol=1e-7, guess=guess)
+    assert pk.tkhp_profile_read_build(P.ctx)["barrier_timeouts"] == 0
+    t0 = time.perf_counter()
+    mu_p, it_p, rms_p = P.polar_solve(Eg, tol=1e-7, guess=guess)
+    waited = time.perf_counter() - t0
+    assert 1.9 < waited < 30.0, waited                       # the barrier's time bound is a time, not a poll count
+    assert pk.tkhp_profile_read_build(P.ctx)["barrier_timeouts"] == 1
+    assert it_p == it_qg and rms_p < 1e-7
+    # ATOM lists: one writer per atom, bit-reproducible; TILES: FP64 atomics, order-dependent last bits
+    same = (lambda a, b: np.array_equal(a, b)) if kernel == "k_pcg_persist" else (lambda a, b: _rel_l2(a, b) < 1e-9)
+    assert same(mu_p.cpu().numpy(), mu_qg.cpu().numpy())
+    _assert_close(mu_p.cpu().numpy(), oracle.dense_solve(s, oracle.perm_field(s)), 1e-5)
+    t0 = time.perf_counter()
+    mu_2, it_2, _ = P.polar_solve(Eg, tol=1e-7)
+    torch.cuda.synchronize()
+    assert time.perf_counter() - t0 < 1.0
+    assert it_2 == it_q and same(mu_2.cpu().numpy(), mu_q.cpu().numpy())
+    assert pk.tkhp_profile_read_build(P.ctx)["barrier_timeouts"] == 1
+    P.close(); Q.close()
+
+
 def test_own_stream_replays_the_build_as_a_graph():
     """On a stream of the caller's (not the legacy default stream) the list build is captured once
     and replayed as a CUDA graph: same lists, same results, also after the inputs change in place
@@ -381,6 +422,36 @@ def test_own_stream_replays_the_build_as_a_graph():
         pk.tkhp_nblist_build(P.ctx, d_pos2, d_al, d_g, st)
         perm, pairs = P.nblist_view(st)
         oracle.check_perm(perm, s.pos, s.box)
+        _assert_close(P.tmatvec(mu, stream=st).cpu().numpy(), oracle.tmatvec(s, mu), 1e-5)
+        # an integrator that alternates between position buffers: both graphs stay cached,
+        # every build is a replay, and each replay reads the buffer it was captured with
+        base = pk.tkhp_profile_read_build(P.ctx)
+        assert base == dict(graph_captures=2, graph_replays=5, plain_builds=0, graphs_off=False, barrier_timeouts=0)
+        for rep in range(6):
+            buf, want = (d_pos, moved) if rep % 2 == 0 else (d_pos2, s.pos)
+            pk.tkhp_nblist_build(P.ctx, buf, d_al, d_g, st)
+            if rep >= 4:
+                perm, pairs = P.nblist_view(st)
+                oracle.check_perm(perm, want, s.box)
+                assert np.array_equal(pairs, oracle.block_pairs(perm, want, s.box, s.cutoff + s.skin))
+        now = pk.tkhp_profile_read_build(P.ctx)
+        assert now == dict(graph_captures=2, graph_replays=11, plain_builds=0, graphs_off=False, barrier_timeouts=0)
+        # more pointer triples than slots: the least recently used graph is replaced, results stay right
+        extra = [torch.as_tensor(s.pos, device="cuda") for _ in range(4)]
+        for buf in extra:
+            pk.tkhp_nblist_build(P.ctx, buf, d_al, d_g, st)
+        pk.tkhp_nblist_build(P.ctx, d_pos, d_al, d_g, st)          # evicted by now: captured again
+        perm, pairs = P.nblist_view(st)
+        oracle.check_perm(perm, moved, s.box)
+        assert np.array_equal(pairs, oracle.block_pairs(perm, moved, s.box, s.cutoff + s.skin))
+        assert pk.tkhp_profile_read_build(P.ctx) == dict(graph_captures=7, graph_replays=16, plain_builds=0,
+                                                         graphs_off=False, barrier_timeouts=0)
+        # the legacy default stream cannot be captured: plain launches, counted as such
+        torch.cuda.synchronize()
+        pk.tkhp_nblist_build(P.ctx, d_pos2, d_al, d_g, 0)
+        perm, pairs = P.nblist_view(0)
+        oracle.check_perm(perm, s.pos, s.box)
+        assert pk.tkhp_profile_read_build(P.ctx)["plain_builds"] == 1
         _assert_close(P.tmatvec(mu, stream=st).cpu().numpy(), oracle.tmatvec(s, mu), 1e-5)
         P.close()
 
@@ -436,6 +507,8 @@ def test_fixed_point_mode_matches_the_oracle(name, list_mode):
     assert abs(e_g - e_ref) <= 1e-6 * abs(e_ref)
     scaled = e_g * float(1 << oracle.FIX_ENERGY_BITS)
     assert scaled == np.rint(scaled) and int(oracle.to_fixed(e_g, oracle.FIX_ENERGY_BITS)) == int(scaled)
+    # one conversion per atom (Q21): from the same arrays the oracle's fixed-point energy is the same integer
+    assert e_g == oracle.polar_energy_fixed(mu_g.cpu().numpy(), Eg.cpu().numpy())
     P.close()
 
 
