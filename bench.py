@@ -66,6 +66,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-stored-t", action="store_true", help="skip the stored-matrix-elements leg (TKHP_SOLVER_STORED_T)")
     ap.add_argument("--peak-seconds", type=float, default=1.0)
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the short legs on configs 0, 1, 3 (MIXED) and config 2 in FP64 / FIXED")
+    ap.add_argument("--other-steps", type=int, default=10, help="timed steps of each short leg")
     ap.add_argument("--table", action="store_true",
                     help="instead of the JSON line: the markdown result table of BASELINE.md section 3 "
                          "(every config and precision, errors against the oracle; several minutes)")
@@ -545,8 +548,83 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         e2e = {"value": replicas.aggregate_throughput(n_pair * (2 + statistics.mean(e2e_iters)), world, e2e_step),
                "unit": UNIT,
                "ms_per_step": e2e_step,
+               "ms_per_step_stats": stats(e2e_ms),
                "h2d_bytes_per_step": n * (24 + 8 + 4 + 8 + 24 + 48),
                "d2h_bytes_per_step": n * 24 + 8}
+
+    # ---- short legs on the other north_star systems and precisions (same step, same timing rules, L2 flushed;
+    # BASELINE.json configs[0], [1], [3] in MIXED and the headline system in FP64 and FIXED), so that the
+    # driver's one line carries them: ms per step, phases, iterations and the dominant kernel's fraction
+    def short_leg(cfg, prec_name, steps):
+        s2 = sys_ if cfg == args.config else make_config(cfg)
+        prec2 = {"mixed": pk.TKHP_MIXED, "fp64": pk.TKHP_FP64, "fixed": pk.TKHP_FIXED}[prec_name]
+        Q = pk.Polarizer.for_system(s2, precision=prec2, list_mode=pk.TKHP_LIST_ATOM, device=local_rank)
+        n2 = s2.n_atoms
+        t_ = lambda a, dt=f64: torch.as_tensor(a, dtype=dt, device=dev)
+        a_pos, a_al, a_g = t_(s2.pos), t_(s2.polarizability), t_(s2.group_id, torch.int32)
+        a_q, a_d, a_th = t_(s2.charge), t_(s2.dipole), t_(s2.quad)
+        o_f = torch.empty((n2, 3), dtype=f64, device=dev)
+        o_mu = torch.empty((n2, 3), dtype=f64, device=dev)
+        o_e = torch.empty((), dtype=f64, device=dev)
+
+        def one():
+            pk.tkhp_nblist_build(Q.ctx, a_pos, a_al, a_g, stream)
+            pk.tkhp_perm_field(Q.ctx, a_q, a_d, a_th, o_f, stream)
+            it_, rms_, _ = pk.tkhp_polar_solve(Q.ctx, o_f, o_mu, args.tol, 100, False, stream)
+            pk.tkhp_polar_energy(Q.ctx, o_mu, o_f, o_e, stream)
+            return it_
+        for _ in range(3):
+            one()
+        torch.cuda.synchronize()
+        np2, ns2, mode2 = Q.nblist_stats()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        tot = dict(n_tmatvec=0, tmatvec_ms=0.0, n_solve=0, solve_ms=0.0, solve_matvecs=0, launches=0)
+        its, phs = [], []
+        pk.tkhp_profile_reset(Q.ctx, True)
+        for k in range(steps):
+            flush.fill_(k & 0xFF)
+            evs[k][0].record(stream)
+            its.append(one())
+            evs[k][1].record(stream)
+            pr_ = pk.tkhp_profile_read(Q.ctx)
+            pr_.update(pk.tkhp_profile_read_solve(Q.ctx))
+            for key in tot:
+                tot[key] += pr_[key]
+            phs.append(Q.timings())
+            pk.tkhp_profile_reset(Q.ctx, True)
+        torch.cuda.synchronize()
+        ms = [a_.elapsed_time(b_) for a_, b_ in evs]
+        if tot["n_solve"] > 0:
+            k_ms = tot["solve_ms"] / tot["n_solve"]
+            mv = tot["solve_matvecs"] / tot["n_solve"]
+            k_name = "k_pcg_persist" if mode2 == pk.TKHP_LIST_ATOM else "k_pcg_tiles"
+        else:
+            k_ms = tot["tmatvec_ms"] / max(tot["n_tmatvec"], 1)
+            mv = 1.0
+            k_name = "T.mu pair kernel (%s list)" % mode_name[mode2]
+        pk2 = peak32 / 2 if prec_name == "fp64" else peak32
+        tf = FLOPS_PER_PAIR_TMU * np2 * mv / (k_ms * 1e-3) / 1e12 if k_ms > 0 else 0.0
+        n_mv = statistics.mean(its) + 1
+        out = {"workload": WORKLOADS[cfg], "precision": prec_name, "n_atoms": n2, "list_mode": mode_name[mode2],
+               "steps": steps, "ms_per_step": statistics.mean(ms), "ms_per_step_stats": stats(ms),
+               "phase_ms": {nm: statistics.mean(ph[nm] for ph in phs) for nm in ("build", "field", "solve", "energy")},
+               "pcg_iterations": statistics.mean(its), "n_pair_within_cutoff": np2,
+               "value": np2 * (1 + n_mv) / (statistics.mean(ms) * 1e-3), "unit": UNIT,
+               "dominant_kernel": k_name, "dominant_kernel_avg_ms": k_ms, "matvecs_per_launch": mv,
+               "dominant_kernel_tflops": tf, "dominant_kernel_frac": tf / pk2, "peak": pk2,
+               "gpu_launches": tot["launches"], "energy_kcal_mol": float(o_e.cpu())}
+        Q.close()
+        return out
+
+    other_configs = None
+    if rank == 0 and world == 1 and not args.no_other_configs and args.config == 2 and args.precision == "mixed":
+        other_configs = []
+        for cfg, prec_name in ((0, "mixed"), (1, "mixed"), (3, "mixed"), (2, "fp64"), (2, "fixed")):
+            try:
+                other_configs.append(short_leg(cfg, prec_name, args.other_steps))
+            except Exception as exc:        # a leg that fails is reported, it does not take the headline down
+                other_configs.append({"workload": WORKLOADS[cfg], "precision": prec_name, "error": repr(exc)})
+            torch.cuda.empty_cache()
 
     # ---- measured FMA peak and the CPU oracle beside it (rank 0, N = 1 only for the oracle)
     fma_peak = pk.tkhp_fma_peak(local_rank, precision, args.peak_seconds) if rank == 0 else None
@@ -586,6 +664,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         "launch_bound": n < 5000,
         "wall_ms_per_step_incl_flush": 1e3 * wall_s / args.steps,
         "roofline": roofline, "stored_t": stored_t, "cpu_baseline": cpu, "e2e": e2e,
+        "other_configs": other_configs,
         "gpu_launches": prof_tot["launches"], "clocks": clocks,
     }
     print(json.dumps(line), flush=True)

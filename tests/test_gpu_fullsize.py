@@ -271,6 +271,50 @@ def test_cfg4_cutoff_sweep(cutoff, precision):
     P.close()
 
 
+_CFG4_ORACLE = {}
+
+
+def _cfg4_oracle(cutoff):
+    """Config 4's FP64 oracle solution at one cutoff (field on every row, PCG to 1e-10: 1-2 minutes of
+    host time), computed once per cutoff for the four library variants below."""
+    if cutoff not in _CFG4_ORACLE:
+        s = make_config(4, cutoff=cutoff)
+        E = oracle.perm_field(s)
+        mu, _, rms = oracle.pcg_solve(s, E, tol=1e-10)
+        assert rms < 1e-10
+        _, it6, _ = oracle.pcg_solve(s, E, tol=1e-6)
+        _CFG4_ORACLE[cutoff] = dict(s=s, E=E, mu=mu, e_pol=oracle.polar_energy(mu, E), it6=it6)
+    return _CFG4_ORACLE[cutoff]
+
+
+@pytest.mark.parametrize("variant", ["mixed", "fp64", "fixed", "stored_t"])
+@pytest.mark.parametrize("cutoff", [9.0, 12.0])
+def test_cfg4_solution_against_the_oracle(cutoff, variant):
+    """BASELINE.json configs[4] asks for the "error versus the FP64 oracle": mu on EVERY row and E_pol against
+    oracle.pcg_solve(tol=1e-10) at 9 and 12 A, at config 2's bars (MIXED 1e-5 / 1e-6, FP64 1e-8 / 1e-9), and the
+    iteration count at 1e-6 against the oracle's.  TKHP_FIXED and TKHP_SOLVER_STORED_T run here on the paths
+    no 7 A case reaches: several chunks per group, so one launch per product instead of the persistent kernel."""
+    import paper_2011_01207_b200 as pk
+    ref = _cfg4_oracle(cutoff)
+    s = ref["s"]
+    prec = {"mixed": pk.TKHP_MIXED, "fp64": pk.TKHP_FP64, "fixed": pk.TKHP_FIXED, "stored_t": pk.TKHP_MIXED}[variant]
+    P = pk.Polarizer.for_system(s, precision=prec, list_mode=pk.TKHP_LIST_ATOM,
+                                solver_flags=pk.TKHP_SOLVER_STORED_T if variant == "stored_t" else 0)
+    P.nblist_build(s.pos, s.polarizability, s.group_id)
+    assert P.nblist_stats(count_pairs=False)[2] == pk.TKHP_LIST_ATOM
+    f64 = variant == "fp64"
+    Eg = P.perm_field(s.charge, s.dipole, s.quad)
+    _assert_close(Eg.cpu().numpy(), ref["E"], 1e-11 if f64 else 1e-5)
+    mu_g, it, rms = P.polar_solve(Eg, tol=1e-12 if f64 else 1e-8)
+    assert rms < (1e-12 if f64 else 1e-8)
+    _assert_close(mu_g.cpu().numpy(), ref["mu"], 1e-8 if f64 else 1e-5)
+    e_g = float(P.polar_energy(mu_g, Eg).cpu())
+    assert abs(e_g - ref["e_pol"]) <= (1e-9 if f64 else 1e-6) * abs(ref["e_pol"])
+    _, it6, rms6 = P.polar_solve(Eg, tol=1e-6)
+    assert it6 == ref["it6"] and rms6 < 1e-6
+    P.close()
+
+
 def test_cfg2_fixed_point_mode(cfg2, cfg2_oracle):
     """Config 2 in the paper's FP mode (TKHP_FIXED): every row against the oracle at the
     MIXED bars, through the persistent solve kernel."""
